@@ -1,0 +1,614 @@
+/*
+ * nyxrt_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, single-threaded fp64 CPU statement of ONE adaptive ray-tracing step on a
+ * uniform coarse grid, written from the paper (arxiv 2512.12466, text at
+ * /root/reference/PAPER.md; "PAPER.md:<line>" below) with the readings R1..R27 recorded in
+ * DESIGN.md ("Readings").  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference leg may load this file.  It shares no code, header, table or helper with the
+ * CUDA library under paper_2512_12466_b200/csrc and neither includes the other.
+ *
+ * Order of the step ("Ray tracing loop", 311 "collect ... duplicates ...
+ * sorted", 313-333 + Alg. 3 at 343-391 "source merging"):
+ *   orc_prepare_sources   dedup same-cell sources, sort
+ *   orc_bubble_radius     MAX_RADIUS of Alg. 3
+ *   orc_merge             MERGE_SOURCES of Alg. 3
+ *   orc_trace             spawn 12 HEALPix rays per source; march / deposit / filter / split
+ *                         depth-first until no ray is left                  (PAPER.md:111-128,
+ *                         152-199, 83-95 Eq. 1-2, 211-249 Eq. 5-8)
+ *   orc_step              the four above in order.
+ *
+ * Traversal is depth-first and recursive (a split recurses into the four children), which is
+ * structurally unlike the CUDA library's pooled breadth-first loop.
+ *
+ * Floating point: everything is IEEE binary64; compile with -O2 -ffp-contract=off and no
+ * fast-math.  fma() is used only where DESIGN.md writes fma.  Expressions that steer control
+ * flow ("DEC" in DESIGN.md) are written exactly in the association DESIGN.md gives.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): HEALPix ring heights / populations and the
+ * inverse map ang->pix (Gorski et al. 2005, PAPER.md:613 ref [63]); slab-method exit distance and
+ * fine-sampled cell lists for the DDA; tau closed form (Eq. 2); photon budget; thin-limit
+ * Gamma = sigma Ndot exp(-tau) / (4 pi R^2) (Eq. 1 with V_shell); Stroemgren I-front, Eq. 10-11
+ * with Table 1 Test A; Eq. 5-8 special cases; split radii from Eq. 4;
+ * brute-force O(N^2)+DFS merge.  Parity UNPINNED by the paper (no printed values): the bubble
+ * sample pattern and the merge defaults (PAPER.md:315-333 leave them to the user), and the
+ * figures 3, 4, 8c.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_OK        0
+#define ORC_EINVAL   -1
+#define ORC_ENOMEM   -3
+#define ORC_EOVERFLOW -5
+
+#define ORC_MAXLEV 16
+
+typedef struct {
+    int32_t nx, ny, nz;
+    int32_t field_dtype;      /* 0 = double fields, 1 = float fields (converted on load, exact) */
+    double  dx_cm;            /* cubic cell width */
+    double  box_lo[3];        /* low corner of cell (0,0,0), in position units */
+    double  pos_unit_cm;      /* cm per position unit */
+} orc_grid;
+
+typedef struct {
+    double  sigma_cm2;        /* monochromatic cross-section                                  */
+    double  n_min_ray;        /* N_min^ray of Eq. 4                         */
+    double  tau_max;          /* RAY_FLTR threshold                             */
+    double  n_th;             /* Eq. 7-8 threshold                          */
+    double  e_excess_erg;     /* heating per photo-ionisation (reading H1)                     */
+    double  automerge_xmean;
+    double  delta_r, r_max, f_ov, x_th, f_req, eps;   /* Alg. 3             */
+    int32_t level_max;        /* l_max of RAY_FLTR                                             */
+    int32_t geom_mode;        /* 0 none, 1 Eq.5 only, 2 Eq.5-6, 3 Eq.7-8, 4 squared [59]       */
+    int32_t merge;            /* 0 off, 1 on, 2 automerge                                      */
+    int32_t n_min_samples;    /* N_min of PAPER.md:317                                         */
+    int32_t samp_level;       /* HEALPix level of the shell sample pattern (reading R6)        */
+    int32_t pad_;
+} orc_params;
+
+typedef struct {
+    uint64_t spawned[ORC_MAXLEV], split[ORC_MAXLEV], killed_tau[ORC_MAXLEV], exited[ORC_MAXLEV],
+             killed_lmax[ORC_MAXLEV];
+    uint64_t segments, zero_len_segments;
+    uint64_t n_src_in, n_src_dedup, n_src_merged;
+    double   photons_emitted, photons_absorbed, photons_escaped, photons_residual, photons_lost;
+} orc_stats;
+
+/* one record per ray-cell segment, optional (tests only) */
+typedef struct {
+    int32_t src, level;
+    int64_t pix;
+    int32_t cell[3];          /* absolute cell of the segment */
+    int32_t nb_face;          /* 0..5 = x-,x+,y-,y+,z-,z+ if the neighbour got a share, else -1 */
+    double  s0, ds, dtau, dN, fc, d_edge, l_pix;
+} orc_seg;
+
+/* ------------------------------------------------------------------------------------------ */
+/* fields                                                                                      */
+
+static inline double fld(const void *p, int dtype, int64_t i) {
+    return dtype ? (double)((const float *)p)[i] : ((const double *)p)[i];
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O2: HEALPix nested pixel centre -> unit vector, "DIR-SPEC".                      */
+/* Pixel geometry: Gorski et al. 2005 (PAPER.md:613 [63]); nested children of p are 4p..4p+3    */
+/* ("splits into four HEALPix subpixels").                                        */
+
+static double sin_poly(double x) {          /* Taylor through x^17, Horner, one fma per step  */
+    double u = x * x, f = 1.0, c[9];
+    int n = 1;
+    for (int k = 0; k < 9; ++k) {           /* c[k] = (-1)^k / (2k+1)!  (division is exact-rounded) */
+        c[k] = ((k & 1) ? -1.0 : 1.0) / f;
+        f = f * (double)(n + 1) * (double)(n + 2);
+        n += 2;
+    }
+    double p = c[8];
+    for (int k = 7; k >= 0; --k) p = fma(p, u, c[k]);
+    return x * p;
+}
+
+static double cos_poly(double x) {          /* Taylor through x^18 */
+    double u = x * x, f = 1.0, c[10];
+    int n = 0;
+    for (int k = 0; k < 10; ++k) {          /* c[k] = (-1)^k / (2k)! */
+        c[k] = ((k & 1) ? -1.0 : 1.0) / f;
+        f = f * (double)(n + 1) * (double)(n + 2);
+        n += 2;
+    }
+    double q = c[9];
+    for (int k = 8; k >= 0; --k) q = fma(q, u, c[k]);
+    return q;
+}
+
+int orc_pix2dir(int level, int64_t pix, double *d) {
+    if (level < 0 || level > 14) return ORC_EINVAL;
+    int64_t ns = (int64_t)1 << level, npf = ns * ns;
+    if (pix < 0 || pix >= 12 * npf) return ORC_EINVAL;
+    int64_t f = pix / npf, pf = pix % npf;
+    int64_t row = f / 4;
+    int64_t ix = 0, iy = 0;
+    for (int b = 0; b < level; ++b) {
+        ix |= ((pf >> (2 * b)) & 1) << b;
+        iy |= ((pf >> (2 * b + 1)) & 1) << b;
+    }
+    int64_t jr = (row + 2) * ns - ix - iy - 1;        /* ring, 1-based from the north pole */
+    int64_t nr, k;
+    double z, st;
+    if (jr < ns) {                                    /* north cap */
+        nr = jr; k = 0;
+        double t = (double)(nr * nr) / (double)(3 * ns * ns);
+        z = 1.0 - t;
+        st = sqrt(t * (2.0 - t));
+    } else if (jr > 3 * ns) {                         /* south cap */
+        nr = 4 * ns - jr; k = 0;
+        double t = (double)(nr * nr) / (double)(3 * ns * ns);
+        z = t - 1.0;
+        st = sqrt(t * (2.0 - t));
+    } else {                                          /* equatorial belt */
+        nr = ns; k = (jr - ns) & 1;
+        z = ((double)(2 * ns - jr) * 2.0) / (double)(3 * ns);
+        st = sqrt((1.0 - z) * (1.0 + z));
+    }
+    int64_t jf = 2 * (f % 4) + (row == 1 ? 0 : 1);
+    int64_t jp = (jf * nr + ix - iy + 1 + k) / 2;
+    if (jp > 4 * nr) jp -= 4 * nr;
+    if (jp < 1) jp += 4 * nr;
+    int64_t m = 2 * jp - k - 1;                       /* phi = (pi/4) m / nr, 0 <= m < 8 nr */
+    int64_t q = m / nr, rem = m % nr;
+    int64_t num = (q & 1) ? (nr - rem) : rem;
+    const double PI_4 = 0x1.921fb54442d18p-1;
+    double alpha = (PI_4 * (double)num) / (double)nr;
+    double c = cos_poly(alpha), s = sin_poly(alpha);
+    if (num == nr) c = s = 0x1.6a09e667f3bcdp-1;       /* phi on a diagonal: cos = sin = sqrt(1/2) exactly alike */
+    double cp, sp;
+    switch ((int)q) {
+        case 0: cp = c;  sp = s;  break;
+        case 1: cp = s;  sp = c;  break;
+        case 2: cp = -s; sp = c;  break;
+        case 3: cp = -c; sp = s;  break;
+        case 4: cp = -c; sp = -s; break;
+        case 5: cp = -s; sp = -c; break;
+        case 6: cp = s;  sp = -c; break;
+        default: cp = c; sp = -s; break;
+    }
+    d[0] = st * cp;
+    d[1] = st * sp;
+    d[2] = z;
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O1: source preparation ("duplicates (sources assigned to the same grid cell)     */
+/* are identified and merged by summing their fluxes. The resulting deduplicated list is then    */
+/* sorted"; "S has integer coords").                                               */
+
+typedef struct { int64_t key; int64_t idx; } keyidx;
+
+static int cmp_keyidx(const void *a, const void *b) {
+    const keyidx *x = a, *y = b;
+    if (x->key != y->key) return x->key < y->key ? -1 : 1;
+    return x->idx < y->idx ? -1 : (x->idx > y->idx);
+}
+
+/* out_cell: [n][3] int32, out_L: [n]; returns count in *n_out (<= n) */
+int orc_prepare_sources(const orc_grid *g, int64_t n, const double *pos, const double *L,
+                        int32_t *out_cell, double *out_L, int64_t *n_out) {
+    *n_out = 0;
+    if (n < 0) return ORC_EINVAL;
+    if (n == 0) return ORC_OK;
+    keyidx *ki = malloc((size_t)n * sizeof *ki);
+    if (!ki) return ORC_ENOMEM;
+    for (int64_t a = 0; a < n; ++a) {
+        int64_t c[3];
+        int32_t dim[3] = { g->nx, g->ny, g->nz };
+        if (!(L[a] >= 0.0) || isinf(L[a])) { free(ki); return ORC_EINVAL; }
+        for (int ax = 0; ax < 3; ++ax) {
+            double u = (pos[3 * a + ax] - g->box_lo[ax]) * g->pos_unit_cm / g->dx_cm;
+            if (!(u >= 0.0) || !(u < (double)dim[ax])) { free(ki); return ORC_EINVAL; }
+            c[ax] = (int64_t)floor(u);
+            if (c[ax] >= dim[ax]) { free(ki); return ORC_EINVAL; }
+        }
+        ki[a].key = (c[2] * g->ny + c[1]) * (int64_t)g->nx + c[0];
+        ki[a].idx = a;
+    }
+    qsort(ki, (size_t)n, sizeof *ki, cmp_keyidx);       /* (key, input index): stable by construction */
+    int64_t m = 0;
+    for (int64_t a = 0; a < n;) {
+        int64_t b = a;
+        double sum = 0.0;
+        while (b < n && ki[b].key == ki[a].key) { sum = sum + L[ki[b].idx]; ++b; }  /* input order */
+        int64_t key = ki[a].key;
+        out_cell[3 * m + 0] = (int32_t)(key % g->nx);
+        out_cell[3 * m + 1] = (int32_t)((key / g->nx) % g->ny);
+        out_cell[3 * m + 2] = (int32_t)(key / ((int64_t)g->nx * g->ny));
+        out_L[m] = sum;
+        ++m;
+        a = b;
+    }
+    free(ki);
+    *n_out = m;
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* M1-M4: MAX_RADIUS (Alg. 3; text 313-319).                                   */
+
+static int in_box(const orc_grid *g, int64_t i, int64_t j, int64_t k) {
+    return i >= 0 && i < g->nx && j >= 0 && j < g->ny && k >= 0 && k < g->nz;
+}
+
+static int64_t lin(const orc_grid *g, int64_t i, int64_t j, int64_t k) {
+    return (k * g->ny + j) * (int64_t)g->nx + i;
+}
+
+int orc_bubble_radius(const orc_grid *g, const orc_params *p, const void *xHI, int64_t n,
+                      const int32_t *cell, double *r_out) {
+    if (p->samp_level < 0 || p->samp_level > 8 || !(p->delta_r > 0.0)) return ORC_EINVAL;
+    int64_t ns = (int64_t)12 << (2 * p->samp_level);
+    double *dir = malloc((size_t)ns * 3 * sizeof *dir);
+    if (!dir) return ORC_ENOMEM;
+    for (int64_t q = 0; q < ns; ++q) orc_pix2dir(p->samp_level, q, dir + 3 * q);
+    for (int64_t a = 0; a < n; ++a) {
+        const int32_t *c = cell + 3 * a;
+        double x0 = 1.0 - fld(xHI, g->field_dtype, lin(g, c[0], c[1], c[2]));  /* ionised fraction */
+        if (x0 < p->x_th) { r_out[a] = 0.0; continue; }
+        double r = p->delta_r, res = -1.0;
+        while (r <= p->r_max) {
+            int64_t ntot = 0, nion = 0;
+            for (int64_t q = 0; q < ns; ++q) {
+                int64_t i = c[0] + (int64_t)floor(fma(r, dir[3 * q + 0], 0.5));
+                int64_t j = c[1] + (int64_t)floor(fma(r, dir[3 * q + 1], 0.5));
+                int64_t k = c[2] + (int64_t)floor(fma(r, dir[3 * q + 2], 0.5));
+                if (!in_box(g, i, j, k)) continue;                            /* "checked" samples */
+                ++ntot;
+                double x = 1.0 - fld(xHI, g->field_dtype, lin(g, i, j, k));
+                if (x >= p->x_th) ++nion;
+            }
+            int pass;
+            if (ntot == 0) pass = 0;                                          /* reading R7 */
+            else if (ntot < p->n_min_samples) pass = (nion == ntot);
+            else pass = ((double)nion >= p->f_req * (double)ntot);
+            if (!pass) { res = r - p->delta_r; break; }
+            r = r + p->delta_r;
+        }
+        r_out[a] = (res >= 0.0) ? res : p->r_max;
+    }
+    free(dir);
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* M5-M8: MERGE_SOURCES (Alg. 3; text 321-333).  All pairs, union-find.        */
+
+static int64_t uf_find(int64_t *par, int64_t a) {
+    while (par[a] != a) { par[a] = par[par[a]]; a = par[a]; }
+    return a;
+}
+
+typedef struct { int64_t key; int32_t c[3]; double L, r; } msrc;
+
+static int cmp_msrc(const void *a, const void *b) {
+    const msrc *x = a, *y = b;
+    return x->key < y->key ? -1 : (x->key > y->key);
+}
+
+int orc_merge(const orc_grid *g, const orc_params *p, int64_t n, const int32_t *cell,
+              const double *L, const double *r, int32_t *out_cell, double *out_L, double *out_r,
+              int64_t *n_out) {
+    *n_out = 0;
+    if (n <= 0) return n < 0 ? ORC_EINVAL : ORC_OK;
+    int64_t *par = malloc((size_t)n * sizeof *par);
+    int64_t *minm = malloc((size_t)n * sizeof *minm);
+    msrc *out = malloc((size_t)n * sizeof *out);
+    if (!par || !minm || !out) { free(par); free(minm); free(out); return ORC_ENOMEM; }
+    for (int64_t a = 0; a < n; ++a) par[a] = a;
+    for (int64_t a = 0; a < n; ++a) {
+        if (!(r[a] > 0.0)) continue;
+        for (int64_t b = a + 1; b < n; ++b) {
+            if (!(r[b] > 0.0)) continue;
+            int64_t dx = (int64_t)cell[3 * a] - cell[3 * b], dy = (int64_t)cell[3 * a + 1] - cell[3 * b + 1],
+                    dz = (int64_t)cell[3 * a + 2] - cell[3 * b + 2];
+            int64_t d2 = dx * dx + dy * dy + dz * dz;
+            double rs = p->f_ov * (r[a] + r[b]);
+            if ((double)d2 <= rs * rs + p->eps) {
+                int64_t ra = uf_find(par, a), rb = uf_find(par, b);
+                if (ra != rb) { if (ra < rb) par[rb] = ra; else par[ra] = rb; }
+            }
+        }
+    }
+    /* smallest member of each component (roots are already the smallest by construction, but do
+       not rely on it) */
+    for (int64_t a = 0; a < n; ++a) minm[a] = n;
+    for (int64_t a = 0; a < n; ++a) { int64_t ra = uf_find(par, a); if (a < minm[ra]) minm[ra] = a; }
+    int64_t m = 0;
+    for (int64_t a = 0; a < n; ++a) {               /* groups in order of their smallest member */
+        int64_t ra = uf_find(par, a);
+        if (minm[ra] != a) continue;
+        int64_t cnt = 0;
+        for (int64_t b = a; b < n; ++b) if (uf_find(par, b) == ra) ++cnt;
+        msrc M;
+        if (cnt == 1) {
+            M.c[0] = cell[3 * a]; M.c[1] = cell[3 * a + 1]; M.c[2] = cell[3 * a + 2];
+            M.L = L[a]; M.r = r[a];
+        } else {
+            double F = 0.0, R = 0.0, num[3] = { 0.0, 0.0, 0.0 };
+            for (int64_t b = a; b < n; ++b) {                                 /* member order */
+                if (uf_find(par, b) != ra) continue;
+                F = F + L[b];
+                if (r[b] > R) R = r[b];
+                for (int ax = 0; ax < 3; ++ax) num[ax] = num[ax] + L[b] * (double)cell[3 * b + ax];
+            }
+            int64_t rc[3];
+            for (int ax = 0; ax < 3; ++ax) rc[ax] = (int64_t)floor(num[ax] / F + 0.5);  /* R9 */
+            int64_t best = -1, bestd = 0;
+            for (int64_t b = a; b < n; ++b) {                                 /* snap */
+                if (uf_find(par, b) != ra) continue;
+                int64_t dx = cell[3 * b] - rc[0], dy = cell[3 * b + 1] - rc[1], dz = cell[3 * b + 2] - rc[2];
+                int64_t d2 = dx * dx + dy * dy + dz * dz;
+                if (best < 0 || d2 < bestd) { best = b; bestd = d2; }         /* first minimum, R10 */
+            }
+            M.c[0] = cell[3 * best]; M.c[1] = cell[3 * best + 1]; M.c[2] = cell[3 * best + 2];
+            M.L = F; M.r = R;
+        }
+        M.key = lin(g, M.c[0], M.c[1], M.c[2]);
+        out[m++] = M;
+    }
+    qsort(out, (size_t)m, sizeof *out, cmp_msrc);                             /* PAPER.md:388; keys unique */
+    for (int64_t a = 0; a < m; ++a) {
+        out_cell[3 * a] = out[a].c[0]; out_cell[3 * a + 1] = out[a].c[1]; out_cell[3 * a + 2] = out[a].c[2];
+        out_L[a] = out[a].L; out_r[a] = out[a].r;
+    }
+    *n_out = m;
+    free(par); free(minm); free(out);
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O3-O7: the ray loop.                                                                          */
+
+typedef struct {
+    const orc_grid *g;
+    const orc_params *p;
+    const void *nH, *xHI;
+    double *gamma, *heat;
+    orc_stats *st;
+    orc_seg *log;
+    int64_t log_cap, log_n;
+    double r2_split[ORC_MAXLEV], K[ORC_MAXLEV];
+    double sdx, V;
+    long double absorbed, escaped, residual, lost;
+    int32_t src_cell[3];
+    int32_t src_id;
+    double L_src;
+} tracer;
+
+static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
+    const orc_grid *g = T->g;
+    const orc_params *p = T->p;
+    orc_stats *st = T->st;
+    const double L_ray = T->L_src / (12.0 * ldexp(1.0, 2 * level));   /* L shared evenly */
+    double d[3], inv[3], sx[3];
+    int64_t o[3];
+    orc_pix2dir(level, pix, d);
+    st->spawned[level]++;
+    /* O4: start-of-life cell in source-relative cell units (source at its cell centre, R3) */
+    for (int a = 0; a < 3; ++a) {
+        double q = fma(s, d[a], 0.5);
+        double fl = floor(q);
+        o[a] = (int64_t)fl;
+        if (q == fl && d[a] < 0.0) o[a] -= 1;                          /* R12 */
+        if (d[a] == 0.0) { inv[a] = 0.0; sx[a] = INFINITY; }
+        else {
+            inv[a] = 1.0 / d[a];
+            sx[a] = ((double)(o[a] + (d[a] > 0.0 ? 1 : 0)) - 0.5) * inv[a];
+        }
+    }
+    if (!in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
+        st->exited[level]++;
+        T->escaped += (long double)(L_ray * exp(-tau));
+        return;
+    }
+    for (;;) {
+        /* 1. kill (RAY_FLTR tau test; per cell, R14) */
+        if (tau >= p->tau_max) {
+            st->killed_tau[level]++;
+            T->residual += (long double)(L_ray * exp(-tau));
+            return;
+        }
+        /* 2. l_max */
+        if (level >= p->level_max) {
+            st->killed_lmax[level]++;
+            T->residual += (long double)(L_ray * exp(-tau));
+            return;
+        }
+        /* 3. split, Eq. 4: Omega_c/Omega(l) < N_min  <=>  s^2 > 3 4^l/(pi N_min) */
+        if (s * s > T->r2_split[level]) {
+            st->split[level]++;
+            for (int k = 0; k < 4; ++k) trace_ray(T, level + 1, 4 * pix + k, s, tau);
+            return;
+        }
+        /* 4. one cell (Amanatides-Woo, PAPER.md:152 [76]) */
+        int ax = 0;
+        double s_exit = sx[0];
+        if (sx[1] < s_exit) { s_exit = sx[1]; ax = 1; }
+        if (sx[2] < s_exit) { s_exit = sx[2]; ax = 2; }                /* first minimum, R19 */
+        double ds = s_exit - s;
+        if (!(ds > 0.0)) ds = 0.0;
+        if (ds > 0.0) {
+            st->segments++;
+            int64_t ci = T->src_cell[0] + o[0], cj = T->src_cell[1] + o[1], ck = T->src_cell[2] + o[2];
+            int64_t c = lin(g, ci, cj, ck);
+            double nH_c = fld(T->nH, g->field_dtype, c);
+            double a_c = nH_c * fld(T->xHI, g->field_dtype, c);        /* absorber density, PAPER.md:229 (R1) */
+            double dtau = (a_c * T->sdx) * ds;                         /* Eq. 2 */
+            double dN = L_ray * exp(-tau) * (-expm1(-dtau));           /* Eq. 1 with V_box */
+            if (dN > 0.0) {
+                double fc = 1.0, d_edge = 0.0, l_pix = 0.0, a_n = 0.0;
+                int face = -1;
+                int64_t cn = -1;                                       /* neighbour that gets a share */
+                if (p->geom_mode != 0) {
+                    /* Sec. 2.6: D_edge = distance from the segment midpoint to the
+                       nearest cell face (R21), L_pix = linear width of the HEALPix pixel there (R22). */
+                    double s_m = s + 0.5 * ds;
+                    double cand[6];
+                    for (int a = 0; a < 3; ++a) {
+                        double m = fma(s_m, d[a], 0.5) - (double)o[a];
+                        if (m < 0.0) m = 0.0;
+                        if (m > 1.0) m = 1.0;
+                        cand[2 * a] = m;                               /* low face  */
+                        cand[2 * a + 1] = 1.0 - m;                     /* high face */
+                    }
+                    face = 0; d_edge = cand[0];
+                    for (int f = 1; f < 6; ++f) if (cand[f] < d_edge) { d_edge = cand[f]; face = f; }
+                    l_pix = s_m * T->K[level];
+                    if (d_edge < 0.5 * l_pix) {                        /* first condition of Eq. 5 / 7 */
+                        if (p->geom_mode == 1) fc = 0.5 + d_edge / l_pix;            /* Eq. 5 alone */
+                        else if (p->geom_mode == 4) { fc = 0.5 + d_edge / l_pix; fc = fc * fc; }  /* [59] */
+                        else {                                         /* 2: Eq. 5-6; 3: Eq. 7-8 */
+                            int64_t nb[3] = { ci, cj, ck };
+                            nb[face >> 1] += (face & 1) ? 1 : -1;
+                            if (in_box(g, nb[0], nb[1], nb[2])) {      /* R23 */
+                                int64_t q = lin(g, nb[0], nb[1], nb[2]);
+                                double nH_n = fld(T->nH, g->field_dtype, q);
+                                a_n = nH_n * fld(T->xHI, g->field_dtype, q);
+                                int ok = a_n > 0.0;                    /* R24 */
+                                if (p->geom_mode == 3 && !(nH_n >= p->n_th)) ok = 0;   /* Eq. 7-8 */
+                                if (ok) { fc = 0.5 + d_edge / l_pix; cn = q; }
+                            }
+                        }
+                    }
+                }
+                double gC = dN / (a_c * T->V);                         /* Gamma of Eq. 1 for this segment */
+                T->gamma[c] += fc * gC;
+                if (T->heat) T->heat[c] += p->e_excess_erg * fc * dN / T->V;       /* H1 */
+                long double dep = (long double)(fc * dN);
+                if (cn >= 0) {
+                    double fn = (1.0 - fc) * (a_c / a_n);              /* Eq. 6 / Eq. 8: f_c' */
+                    T->gamma[cn] += fn * gC;
+                    if (T->heat) T->heat[cn] += p->e_excess_erg * (1.0 - fc) * dN / T->V;
+                    dep += (long double)((1.0 - fc) * dN);
+                } else if (fc < 1.0) {
+                    T->lost += (long double)((1.0 - fc) * dN);         /* modes 1, 4 */
+                }
+                T->absorbed += dep;
+                if (T->log && T->log_n < T->log_cap) {
+                    orc_seg *r = &T->log[T->log_n];
+                    r->src = T->src_id; r->level = level; r->pix = pix;
+                    r->cell[0] = (int32_t)ci; r->cell[1] = (int32_t)cj; r->cell[2] = (int32_t)ck;
+                    r->nb_face = (cn >= 0) ? face : -1;
+                    r->s0 = s; r->ds = ds; r->dtau = dtau; r->dN = dN; r->fc = fc;
+                    r->d_edge = d_edge; r->l_pix = l_pix;
+                }
+                if (T->log) T->log_n++;
+            } else if (T->log) {
+                if (T->log_n < T->log_cap) {
+                    orc_seg *r = &T->log[T->log_n];
+                    memset(r, 0, sizeof *r);
+                    r->src = T->src_id; r->level = level; r->pix = pix;
+                    r->cell[0] = (int32_t)ci; r->cell[1] = (int32_t)cj; r->cell[2] = (int32_t)ck;
+                    r->nb_face = -1; r->s0 = s; r->ds = ds; r->dtau = dtau; r->fc = 1.0;
+                }
+                T->log_n++;
+            }
+            tau = tau + dtau;
+        } else {
+            st->zero_len_segments++;
+        }
+        s = s_exit;
+        o[ax] += (d[ax] > 0.0) ? 1 : -1;
+        sx[ax] = ((double)(o[ax] + (d[ax] > 0.0 ? 1 : 0)) - 0.5) * inv[ax];
+        if (!in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
+            st->exited[level]++;                                        /* R20 */
+            T->escaped += (long double)(L_ray * exp(-tau));
+            return;
+        }
+    }
+}
+
+/* gamma, heat: [nz][ny][nx] double, overwritten.  heat may be NULL.  log may be NULL.
+   *log_n_out (may be NULL) receives the number of segments that WOULD have been logged. */
+int orc_trace(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
+              int64_t n_cat, const int32_t *cell, const double *L, double *gamma, double *heat,
+              orc_stats *st, orc_seg *log, int64_t log_cap, int64_t *log_n_out) {
+    if (p->level_max < 0 || p->level_max >= ORC_MAXLEV - 1 || !(p->n_min_ray > 0.0)) return ORC_EINVAL;
+    if (p->geom_mode < 0 || p->geom_mode > 4) return ORC_EINVAL;
+    int64_t ncell = (int64_t)g->nx * g->ny * g->nz;
+    memset(gamma, 0, (size_t)ncell * sizeof *gamma);
+    if (heat) memset(heat, 0, (size_t)ncell * sizeof *heat);
+    tracer T;
+    memset(&T, 0, sizeof T);
+    T.g = g; T.p = p; T.nH = nH; T.xHI = xHI; T.gamma = gamma; T.heat = heat; T.st = st;
+    T.log = log; T.log_cap = log_cap; T.log_n = 0;
+    const double PI = 0x1.921fb54442d18p+1;
+    for (int l = 0; l < ORC_MAXLEV; ++l) {
+        T.r2_split[l] = ldexp(3.0 / (PI * p->n_min_ray), 2 * l);       /* Eq. 4 */
+        T.K[l] = ldexp(sqrt(PI / 3.0), -l);                            /* sqrt(Omega(l)), R22 */
+    }
+    T.sdx = p->sigma_cm2 * g->dx_cm;
+    T.V = g->dx_cm * g->dx_cm * g->dx_cm;                              /* V_box = h^3 */
+    long double emitted = 0.0L;
+    for (int64_t a = 0; a < n_cat; ++a) {
+        T.src_cell[0] = cell[3 * a]; T.src_cell[1] = cell[3 * a + 1]; T.src_cell[2] = cell[3 * a + 2];
+        if (!in_box(g, T.src_cell[0], T.src_cell[1], T.src_cell[2])) return ORC_EINVAL;
+        T.src_id = (int32_t)a;
+        T.L_src = L[a];
+        emitted += (long double)L[a];
+        for (int64_t pix = 0; pix < 12; ++pix) trace_ray(&T, 0, pix, 0.0, 0.0);
+    }
+    st->photons_emitted = (double)emitted;
+    st->photons_absorbed = (double)T.absorbed;
+    st->photons_escaped = (double)T.escaped;
+    st->photons_residual = (double)T.residual;
+    st->photons_lost = (double)T.lost;
+    if (log_n_out) *log_n_out = T.log_n;
+    return ORC_OK;
+}
+
+/* mean ionised fraction over all cells (automerge trigger) */
+double orc_mean_ionised(const orc_grid *g, const void *xHI) {
+    int64_t ncell = (int64_t)g->nx * g->ny * g->nz;
+    long double s = 0.0L;
+    for (int64_t i = 0; i < ncell; ++i) s += (long double)(1.0 - fld(xHI, g->field_dtype, i));
+    return (double)(s / (long double)ncell);
+}
+
+/* The whole step.  cat_* have room for n_src entries; *n_cat receives the catalogue length. */
+int orc_step(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
+             int64_t n_src, const double *pos, const double *L,
+             double *gamma, double *heat, orc_stats *st,
+             int32_t *cat_cell, double *cat_L, double *cat_r, int64_t *n_cat) {
+    memset(st, 0, sizeof *st);
+    int64_t nd = 0;
+    int rc = orc_prepare_sources(g, n_src, pos, L, cat_cell, cat_L, &nd);
+    if (rc) return rc;
+    st->n_src_in = (uint64_t)n_src;
+    st->n_src_dedup = (uint64_t)nd;
+    for (int64_t a = 0; a < nd; ++a) cat_r[a] = 0.0;
+    int do_merge = p->merge == 1 || (p->merge == 2 && orc_mean_ionised(g, xHI) > p->automerge_xmean);
+    int64_t nm = nd;
+    if (do_merge && nd > 0) {
+        int32_t *c2 = malloc((size_t)nd * 3 * sizeof *c2);
+        double *L2 = malloc((size_t)nd * sizeof *L2), *r2 = malloc((size_t)nd * sizeof *r2);
+        if (!c2 || !L2 || !r2) { free(c2); free(L2); free(r2); return ORC_ENOMEM; }
+        rc = orc_bubble_radius(g, p, xHI, nd, cat_cell, cat_r);
+        if (!rc) rc = orc_merge(g, p, nd, cat_cell, cat_L, cat_r, c2, L2, r2, &nm);
+        if (!rc) {
+            memcpy(cat_cell, c2, (size_t)nm * 3 * sizeof *c2);
+            memcpy(cat_L, L2, (size_t)nm * sizeof *L2);
+            memcpy(cat_r, r2, (size_t)nm * sizeof *r2);
+        }
+        free(c2); free(L2); free(r2);
+        if (rc) return rc;
+    }
+    st->n_src_merged = (uint64_t)nm;
+    *n_cat = nm;
+    return orc_trace(g, p, nH, xHI, nm, cat_cell, cat_L, gamma, heat, st, NULL, 0, NULL);
+}
+
+int orc_sizeof_stats(void) { return (int)sizeof(orc_stats); }
+int orc_sizeof_seg(void) { return (int)sizeof(orc_seg); }

@@ -1,0 +1,211 @@
+"""ctypes front end of the CPU oracle (oracle/nyxrt_oracle.c).  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It never imports the product package, and the product package never imports it.
+Everything here is argument marshalling; the arithmetic is in nyxrt_oracle.c, which cites the paper.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "nyxrt_oracle.c")
+_LIB = os.path.join(_HERE, "libnyxrt_oracle.so")
+MAXLEV = 16
+
+
+def build(force=False):
+    """gcc -O2 -ffp-contract=off (no fast-math): decisions must not be contracted (DESIGN.md DEC)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-Wall",
+                               "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class Grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("field_dtype", C.c_int32),
+                ("dx_cm", C.c_double), ("box_lo", C.c_double * 3), ("pos_unit_cm", C.c_double)]
+
+
+class Params(C.Structure):
+    _fields_ = [("sigma_cm2", C.c_double), ("n_min_ray", C.c_double), ("tau_max", C.c_double),
+                ("n_th", C.c_double), ("e_excess_erg", C.c_double), ("automerge_xmean", C.c_double),
+                ("delta_r", C.c_double), ("r_max", C.c_double), ("f_ov", C.c_double), ("x_th", C.c_double),
+                ("f_req", C.c_double), ("eps", C.c_double),
+                ("level_max", C.c_int32), ("geom_mode", C.c_int32), ("merge", C.c_int32),
+                ("n_min_samples", C.c_int32), ("samp_level", C.c_int32), ("pad_", C.c_int32)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("spawned", C.c_uint64 * MAXLEV), ("split", C.c_uint64 * MAXLEV),
+                ("killed_tau", C.c_uint64 * MAXLEV), ("exited", C.c_uint64 * MAXLEV),
+                ("killed_lmax", C.c_uint64 * MAXLEV),
+                ("segments", C.c_uint64), ("zero_len_segments", C.c_uint64),
+                ("n_src_in", C.c_uint64), ("n_src_dedup", C.c_uint64), ("n_src_merged", C.c_uint64),
+                ("photons_emitted", C.c_double), ("photons_absorbed", C.c_double),
+                ("photons_escaped", C.c_double), ("photons_residual", C.c_double),
+                ("photons_lost", C.c_double)]
+
+    def as_dict(self):
+        d = {}
+        for name, _ in self._fields_:
+            v = getattr(self, name)
+            d[name] = list(v) if hasattr(v, "__len__") else v
+        return d
+
+
+SEG_DTYPE = np.dtype([("src", "<i4"), ("level", "<i4"), ("pix", "<i8"), ("cell", "<i4", (3,)),
+                      ("nb_face", "<i4"), ("s0", "<f8"), ("ds", "<f8"), ("dtau", "<f8"), ("dN", "<f8"),
+                      ("fc", "<f8"), ("d_edge", "<f8"), ("l_pix", "<f8")], align=True)
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_mean_ionised.restype = C.c_double
+        assert _lib.orc_sizeof_stats() == C.sizeof(Stats)
+        assert _lib.orc_sizeof_seg() == SEG_DTYPE.itemsize, (_lib.orc_sizeof_seg(), SEG_DTYPE.itemsize)
+    return _lib
+
+
+def make_grid(shape_zyx, dx_cm, field_dtype=np.float64, box_lo=(0.0, 0.0, 0.0), pos_unit_cm=None):
+    g = Grid()
+    g.nz, g.ny, g.nx = [int(v) for v in shape_zyx]
+    g.field_dtype = 1 if np.dtype(field_dtype) == np.float32 else 0
+    g.dx_cm = float(dx_cm)
+    g.box_lo[:] = [float(v) for v in box_lo]
+    g.pos_unit_cm = float(dx_cm if pos_unit_cm is None else pos_unit_cm)   # default: positions in cells
+    return g
+
+
+def make_params(**kw):
+    """Field names follow the paper's symbols; defaults are DESIGN.md's table of parameters."""
+    d = dict(sigma_cm2=6.3e-18, n_min_ray=3.0, tau_max=float(np.log(1e8)), n_th=0.0, e_excess_erg=0.0,
+             automerge_xmean=0.018, delta_r=2.0, r_max=8.0, f_ov=1.0, x_th=0.9, f_req=0.75, eps=1e-9,
+             level_max=13, geom_mode=3, merge=0, n_min_samples=16, samp_level=2)
+    d.update(kw)
+    p = Params()
+    for k, v in d.items():
+        setattr(p, k, v)
+    return p
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise RuntimeError("oracle %s failed with code %d" % (what, rc))
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def pix2dir(level, pix):
+    out = np.zeros(3)
+    _chk(lib().orc_pix2dir(C.c_int(level), C.c_int64(int(pix)), _ptr(out)), "pix2dir")
+    return out
+
+
+def pix2dir_all(level):
+    n = 12 * 4 ** level
+    out = np.zeros((n, 3))
+    f = lib().orc_pix2dir
+    for p in range(n):
+        f(C.c_int(level), C.c_int64(p), C.c_void_p(out.ctypes.data + 24 * p))
+    return out
+
+
+def prepare_sources(g, pos, L):
+    pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+    L = np.ascontiguousarray(L, dtype=np.float64)
+    n = len(L)
+    cell = np.zeros((max(n, 1), 3), np.int32)
+    Lo = np.zeros(max(n, 1))
+    nout = C.c_int64(0)
+    _chk(lib().orc_prepare_sources(C.byref(g), C.c_int64(n), _ptr(pos), _ptr(L), _ptr(cell), _ptr(Lo),
+                                   C.byref(nout)), "prepare_sources")
+    return cell[:nout.value].copy(), Lo[:nout.value].copy()
+
+
+def _field(g, a):
+    want = np.float32 if g.field_dtype else np.float64
+    a = np.ascontiguousarray(a)
+    assert a.dtype == want, (a.dtype, want)
+    assert a.shape == (g.nz, g.ny, g.nx), (a.shape, (g.nz, g.ny, g.nx))
+    return a
+
+
+def bubble_radius(g, p, xHI, cell):
+    xHI = _field(g, xHI)
+    cell = np.ascontiguousarray(cell, np.int32).reshape(-1, 3)
+    r = np.zeros(len(cell))
+    _chk(lib().orc_bubble_radius(C.byref(g), C.byref(p), _ptr(xHI), C.c_int64(len(cell)), _ptr(cell), _ptr(r)),
+         "bubble_radius")
+    return r
+
+
+def merge(g, p, cell, L, r):
+    cell = np.ascontiguousarray(cell, np.int32).reshape(-1, 3)
+    L = np.ascontiguousarray(L, np.float64)
+    r = np.ascontiguousarray(r, np.float64)
+    n = len(L)
+    oc = np.zeros((max(n, 1), 3), np.int32)
+    oL = np.zeros(max(n, 1))
+    orr = np.zeros(max(n, 1))
+    nout = C.c_int64(0)
+    _chk(lib().orc_merge(C.byref(g), C.byref(p), C.c_int64(n), _ptr(cell), _ptr(L), _ptr(r), _ptr(oc), _ptr(oL),
+                         _ptr(orr), C.byref(nout)), "merge")
+    m = nout.value
+    return oc[:m].copy(), oL[:m].copy(), orr[:m].copy()
+
+
+def trace(g, p, nH, xHI, cell, L, want_heat=True, log_cap=0):
+    """Returns (gamma, heat, stats[, seglog])."""
+    nH = _field(g, nH)
+    xHI = _field(g, xHI)
+    cell = np.ascontiguousarray(cell, np.int32).reshape(-1, 3)
+    L = np.ascontiguousarray(L, np.float64)
+    gamma = np.zeros((g.nz, g.ny, g.nx))
+    heat = np.zeros((g.nz, g.ny, g.nx)) if want_heat else None
+    st = Stats()
+    log = np.zeros(log_cap, SEG_DTYPE) if log_cap else None
+    nlog = C.c_int64(0)
+    _chk(lib().orc_trace(C.byref(g), C.byref(p), _ptr(nH), _ptr(xHI), C.c_int64(len(L)), _ptr(cell), _ptr(L),
+                         _ptr(gamma), _ptr(heat) if want_heat else None, C.byref(st),
+                         _ptr(log) if log_cap else None, C.c_int64(log_cap), C.byref(nlog)), "trace")
+    if log_cap:
+        if nlog.value > log_cap:
+            raise RuntimeError("segment log overflow: %d > %d" % (nlog.value, log_cap))
+        return gamma, heat, st, log[:nlog.value]
+    return gamma, heat, st
+
+
+def step(g, p, nH, xHI, pos, L, want_heat=True):
+    """The whole RT step.  Returns (gamma, heat, stats, (cat_cell, cat_L, cat_r))."""
+    nH = _field(g, nH)
+    xHI = _field(g, xHI)
+    pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+    L = np.ascontiguousarray(L, dtype=np.float64)
+    n = len(L)
+    gamma = np.zeros((g.nz, g.ny, g.nx))
+    heat = np.zeros((g.nz, g.ny, g.nx)) if want_heat else None
+    st = Stats()
+    cc = np.zeros((max(n, 1), 3), np.int32)
+    cL = np.zeros(max(n, 1))
+    cr = np.zeros(max(n, 1))
+    ncat = C.c_int64(0)
+    _chk(lib().orc_step(C.byref(g), C.byref(p), _ptr(nH), _ptr(xHI), C.c_int64(n), _ptr(pos), _ptr(L),
+                        _ptr(gamma), _ptr(heat) if want_heat else None, C.byref(st), _ptr(cc), _ptr(cL), _ptr(cr),
+                        C.byref(ncat)), "step")
+    m = ncat.value
+    return gamma, heat, st, (cc[:m].copy(), cL[:m].copy(), cr[:m].copy())
+
+
+def mean_ionised(g, xHI):
+    return lib().orc_mean_ionised(C.byref(g), _ptr(_field(g, xHI)))
