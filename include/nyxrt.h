@@ -1,0 +1,168 @@
+/*
+ * nyxrt.h -- C ABI of the B200-native adaptive ray-tracing step (one RT step on the coarse grid) of
+ * Nyx-RT, arxiv 2512.12466.  Citations are lines of /root/reference/PAPER.md ("PAPER.md:<line>");
+ * readings R1..R27 and H1 of the paper's silent / garbled spots are listed in DESIGN.md.
+ *
+ * The step ("Ray tracing loop", Figs. 1-2 at PAPER.md:120-124; Sec. 2.8 at 295-391):
+ *   source dedup + sort -> [bubble radius -> merge] -> emit 12 HEALPix rays per source ->
+ *   { march cell by cell and deposit (Eq. 1-2, Eq. 5-8) -> filter -> split into 4 children } until no
+ *   ray is left -> finalise Gamma_HI and the heating rate.
+ *
+ * Conventions
+ *   - Every function returns NYXRT_OK (0) or a negative NYXRT_E* code; the message is available from
+ *     nyxrt_last_error().  Nothing throws, aborts or prints.
+ *   - "device pointer" = CUDA device memory on the context's device; "host pointer" = ordinary host
+ *     memory.  Nothing in a signature is a torch (or any other framework's) type.
+ *   - Grids are dense [nz][ny][nx], x fastest: index = (k*ny + j)*nx + i.
+ *   - Streams are cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - A context is not thread-safe; use one per host thread / per grid.
+ *   - There is no CPU fallback: without a CUDA device nyxrt_create fails with NYXRT_ECUDA.
+ */
+#ifndef NYXRT_H
+#define NYXRT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NYXRT_OK          0
+#define NYXRT_EINVAL     -1   /* bad argument (incl. a source outside the box, L < 0, NaN)         */
+#define NYXRT_ESTATE     -2   /* call order: fields / sources / workspace not set                  */
+#define NYXRT_ENOMEM     -3   /* workspace too small (see nyxrt_workspace_bytes)                   */
+#define NYXRT_ECUDA      -4   /* a CUDA call failed; message holds cudaGetErrorString              */
+#define NYXRT_EOVERFLOW  -5   /* ray pool overflow or HEALPix level > 14; never silent truncation  */
+
+#define NYXRT_MAXLEV 16
+
+typedef struct nyxrt_ctx nyxrt_ctx;      /* opaque */
+
+/* The coarse RT grid ("downsampled onto a coarse grid"; cubic cells). */
+typedef struct {
+    int32_t nx, ny, nz;        /* cells per axis, each 1..2^20 and nx*ny*nz < 2^40                  */
+    int32_t field_dtype;       /* 0 = fp64 fields, 1 = fp32 fields (converted on load, exact)       */
+    double  dx_cm;             /* cell width h in cm; V_box = h^3 (PAPER.md:205 footnote 2)         */
+    double  box_lo[3];         /* position of the low corner of cell (0,0,0), in position units     */
+    double  pos_unit_cm;       /* cm per position unit of nyxrt_set_sources (dx_cm => cell units)    */
+    int32_t periodic;          /* must be 0: rays die on leaving the box (BASELINE.json; R20)       */
+    int32_t device;            /* CUDA device ordinal                                               */
+} nyxrt_grid;
+
+/* User parameters; names follow the paper's symbols.  Defaults: DESIGN.md "Parameters". */
+typedef struct {
+    double  sigma_cm2;         /* monochromatic H I cross-section (6.3e-18)                         */
+    double  n_min_ray;         /* N_min^ray of Eq. 4, PAPER.md:113-116 (3; paper production: 2)     */
+    double  tau_max;           /* RAY_FLTR optical-depth threshold, PAPER.md:128, 174 (ln 1e8)      */
+    double  n_th;              /* low-density neighbour threshold of Eq. 7-8      */
+    double  e_excess_erg;      /* heating per photo-ionisation (reading H1; 0 at 13.6 eV)           */
+    double  automerge_xmean;   /* merge==2: merge once mean ionised fraction exceeds this (0.018)   */
+    double  delta_r;           /* Alg. 3 shell spacing in cells, PAPER.md:313 (2)                   */
+    double  r_max;             /* Alg. 3 R_max in cells                               */
+    double  f_ov;              /* overlap factor                                  */
+    double  x_th;              /* ionised threshold of a sample                       */
+    double  f_req;             /* required ionised share of a shell                   */
+    double  eps;               /* tolerance of the link test                      */
+    int32_t level_max;         /* l_max of RAY_FLTR, PAPER.md:174 (<= 13)                           */
+    int32_t geom_mode;         /* 0 none, 1 Eq.5 only, 2 Eq.5-6, 3 Eq.7-8 (default), 4 squared [59] */
+    int32_t merge;             /* 0 off, 1 on, 2 automerge                           */
+    int32_t n_min_samples;     /* N_min of PAPER.md:317                                             */
+    int32_t samp_level;        /* HEALPix level of the shell sample pattern, 12*4^level dirs (R6)   */
+    int32_t reserved;          /* 0                                                                 */
+} nyxrt_params;
+
+/* Filled by nyxrt_trace (host memory).  Per-level arrays are indexed by HEALPix level l. */
+typedef struct {
+    uint64_t spawned[NYXRT_MAXLEV];      /* rays created at level l (12 per source at l = 0)        */
+    uint64_t split[NYXRT_MAXLEV];        /* rays that met Eq. 4 and became 4 children               */
+    uint64_t killed_tau[NYXRT_MAXLEV];   /* rays filtered by tau >= tau_max                         */
+    uint64_t exited[NYXRT_MAXLEV];       /* rays that left the box                                  */
+    uint64_t killed_lmax[NYXRT_MAXLEV];  /* rays filtered by l >= l_max                             */
+    uint64_t segments;                   /* ray-cell segments of positive length (the work unit)    */
+    uint64_t zero_len_segments;          /* cell crossings of zero length (edge / corner hits)      */
+    uint64_t n_src_in, n_src_dedup, n_src_merged;
+    uint64_t iterations;                 /* march launches (diagnostic; not part of parity)         */
+    uint64_t peak_pool_rays;             /* max rays resident in the pool (diagnostic)              */
+    double   photons_emitted;            /* sum of catalogue L [s^-1]                               */
+    double   photons_absorbed;           /* sum over cells of deposited photons [s^-1]              */
+    double   photons_escaped;            /* carried out of the box                                  */
+    double   photons_residual;           /* left in rays filtered by tau_max / l_max                */
+    double   photons_lost;               /* geom_mode 1 and 4 only (no secondary correction)        */
+    float    ms_sources, ms_loop, ms_finalise, ms_total;   /* CUDA-event times of the phases        */
+} nyxrt_stats;
+
+/* Create a context for one grid.  Copies *grid and *params.  Allocates only small bookkeeping
+ * (host + a few KB device).  Errors: EINVAL (bad sizes / parameters, periodic != 0), ECUDA. */
+int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx **out);
+
+/* Size of the caller-provided device workspace.
+ *   max_sources     upper bound of n in nyxrt_set_sources
+ *   batch_rays      rays marched per launch B (0 = default 2^21); the ray pool holds
+ *                   (2 + 5*(level_max+1)) * B rays of 32 bytes
+ *   host_staging    non-zero: add room for the fields and outputs of nyxrt_step_host
+ * Workspace layout is private.  Errors: EINVAL. */
+int nyxrt_workspace_bytes(const nyxrt_ctx *ctx, int64_t max_sources, int64_t batch_rays, int32_t host_staging,
+                          uint64_t *bytes);
+
+/* Hand the library its workspace (device pointer, 256-byte aligned, owned by the caller, must stay
+ * valid until nyxrt_destroy or the next nyxrt_set_workspace).  The same max_sources / batch_rays /
+ * host_staging as in nyxrt_workspace_bytes.  Errors: EINVAL, ENOMEM (bytes too small). */
+int nyxrt_set_workspace(nyxrt_ctx *ctx, void *d_workspace, uint64_t bytes, int64_t max_sources,
+                        int64_t batch_rays, int32_t host_staging);
+
+/* Register the fields of this step: total hydrogen density n_H [cm^-3] and NEUTRAL fraction x_HI
+ * (absorber density a_abs = x_HI n_H, PAPER.md:229 with x_HI = 1 - x; reading R1), device pointers of
+ * grid.field_dtype, layout [nz][ny][nx].  Borrowed until the next nyxrt_set_fields / nyxrt_destroy.
+ * Enqueues on `stream` the kernel that builds the internal absorber field; does not synchronise.
+ * Values are not validated (n_H < 0, x_HI outside [0,1], NaN: garbage in, garbage out).
+ * Errors: EINVAL (NULL), ESTATE (no workspace), ECUDA. */
+int nyxrt_set_fields(nyxrt_ctx *ctx, const void *d_nH, const void *d_xHI, void *cuda_stream);
+
+/* Set the point sources of this step: host pointers, pos_xyz is [n][3] in
+ * position units, L is [n] photons/s.  Copied; validated on the device: a source outside the box,
+ * L < 0, NaN or inf -> EINVAL and the previous source list is dropped.  Synchronises `stream`.
+ * Errors: EINVAL, ESTATE (no workspace), ENOMEM (n > max_sources), ECUDA. */
+int nyxrt_set_sources(nyxrt_ctx *ctx, int64_t n, const double *pos_xyz, const double *L, void *cuda_stream);
+
+/* Run one RT step.  d_gamma_HI (required) and d_heat (may be NULL) are device pointers to
+ * [nz][ny][nx] doubles, overwritten:
+ *   Gamma_HI [s^-1 per H I atom] = photons absorbed in the cell / (n_HI V)      (Eq. 1)
+ *   heat [erg s^-1 cm^-3]        = e_excess * photons absorbed in the cell / V   (reading H1)
+ * A cell that received nothing holds exactly 0.  All work is enqueued on `stream`; the call
+ * synchronises that stream before filling *h_stats (host pointer, may be NULL).
+ * Errors: ESTATE (fields / sources / workspace missing), EOVERFLOW, ECUDA. */
+int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma_HI, double *d_heat, nyxrt_stats *h_stats, void *cuda_stream);
+
+/* The (deduplicated, merged, sorted) catalogue the last nyxrt_trace used: host
+ * pointers with room for `cap` entries; cell_ijk is [cap][3]; radius is the bubble radius in cells
+ * (0 when merging was off).  Any of the three arrays may be NULL.  *n_out = catalogue length even
+ * when cap is smaller (then only cap entries are written).  Errors: ESTATE, ECUDA. */
+int nyxrt_get_catalog(nyxrt_ctx *ctx, int64_t cap, int32_t *cell_ijk, double *L, double *radius, int64_t *n_out);
+
+/* The same step end to end with HOST buffers: copies the fields and sources to the device, runs
+ * nyxrt_set_fields + nyxrt_set_sources + nyxrt_trace on an internal stream, copies Gamma_HI (and the
+ * heating rate unless h_heat is NULL) back.  Needs a workspace created with host_staging != 0.
+ * Errors: as the three calls. */
+int nyxrt_step_host(nyxrt_ctx *ctx, const void *h_nH, const void *h_xHI, int64_t n_src, const double *pos_xyz,
+                    const double *L, double *h_gamma_HI, double *h_heat, nyxrt_stats *h_stats);
+
+/* HEALPix nested pixel centre of (level, pix) as the library computes it on the device (DIR-SPEC,
+ * DESIGN.md): n directions into the host array dir_xyz [n][3].  For tests.  Errors: EINVAL, ECUDA. */
+int nyxrt_pix2dir(nyxrt_ctx *ctx, int32_t level, int64_t pix_begin, int64_t n, double *dir_xyz);
+
+/* Message of the last failed call on this context ("" if none).  Never NULL. */
+const char *nyxrt_last_error(const nyxrt_ctx *ctx);
+
+/* Free the context (not the workspace, which the caller owns).  NULL is allowed. */
+void nyxrt_destroy(nyxrt_ctx *ctx);
+
+/* Library version and the size of the public structs (for binding self-checks). */
+int nyxrt_version(void);
+int nyxrt_sizeof_grid(void);
+int nyxrt_sizeof_params(void);
+int nyxrt_sizeof_stats(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NYXRT_H */

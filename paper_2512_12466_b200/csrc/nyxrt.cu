@@ -1,0 +1,591 @@
+// C ABI of the B200-native adaptive ray-tracing step (include/nyxrt.h).  Host orchestration only: every
+// step of the path runs in the kernels of march.cuh / sources.cuh (plus CUB radix sort and scan as
+// library primitives inside the source pass).
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_scan.cuh>
+
+#include "../../include/nyxrt.h"
+#include "march.cuh"
+#include "sources.cuh"
+
+using namespace nyxrt;
+
+namespace {
+
+constexpr int NPARTIAL = 2048;            // blocks of the grid-wide reductions (prep, finalise)
+
+struct SrcBufs {
+    double *pos, *L;                       // input sources
+    long long *key_a, *key_b;              // cell keys (unsorted / sorted)
+    int *idx_a, *idx_b, *flag, *gid;       // permutation, run heads, run ids
+    int *par, *lab_a, *lab_b, *bin_a, *bin_b;
+    int4 *cell[2];
+    double *L2[2], *r[2];
+    long long *ckey[2];
+    int *bad;
+    double *dirs;                          // shell sample directions, 12*4^samp_level
+    void *cub_tmp;
+    size_t cub_bytes;
+};
+
+}  // namespace
+
+struct nyxrt_ctx {
+    nyxrt_grid g;
+    nyxrt_params p;
+    char err[512];
+    int sm_count, march_blocks, nlev;
+    long long ncell;
+    // workspace
+    void *ws;
+    uint64_t ws_bytes;
+    long long max_sources, batch_rays;
+    int host_staging;
+    double *absorber, *partial, *scalars;  // scalars[0] = sum(1-x_HI), [1] = absorbed, [2] = emitted
+    RayPool pool;
+    LoopState *ls;
+    DevStats *ds;
+    SrcBufs sb;
+    void *st_nH, *st_xHI;
+    double *st_gamma, *st_heat;
+    // state
+    const void *d_nH, *d_xHI;
+    bool have_fields, have_sources, have_catalog;
+    long long n_src, n_dedup, n_cat;
+    int cat_sel;                           // which of sb.cell[]/L2[]/r[] holds the final catalogue
+    double r2_split[MAXLEV], K[MAXLEV];
+    cudaEvent_t ev[4];
+    cudaStream_t own_stream;
+    LoopState *h_ls;                       // pinned
+    DevStats *h_ds;                        // pinned
+    double *h_scalars;                     // pinned
+};
+
+namespace {
+
+int fail(nyxrt_ctx *c, int code, const char *fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof c->err, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(ctx, NYXRT_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                        __FILE__, __LINE__);                                                       \
+    } while (0)
+
+inline unsigned blocks_for(long long n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+size_t field_elem(const nyxrt_ctx *c) { return c->g.field_dtype ? 4 : 8; }
+
+// bump allocator over the workspace; base == nullptr only measures
+struct Bump {
+    char *base;
+    uint64_t off;
+    template <typename T>
+    T *take(uint64_t n) {
+        off = (off + 255) & ~uint64_t(255);
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+size_t cub_temp_bytes(long long n) {
+    size_t a = 0, b = 0, c = 0;
+    cub::DeviceRadixSort::SortPairs(nullptr, a, (long long *)nullptr, (long long *)nullptr, (int *)nullptr,
+                                    (int *)nullptr, (int)n);
+    cub::DeviceRadixSort::SortPairs(nullptr, b, (int *)nullptr, (int *)nullptr, (int *)nullptr, (int *)nullptr, (int)n);
+    cub::DeviceScan::InclusiveSum(nullptr, c, (int *)nullptr, (int *)nullptr, (int)n);
+    size_t m = a > b ? a : b;
+    return (m > c ? m : c) + 256;
+}
+
+// number of pool levels that can hold rays at all: level l needs s^2 > r2_split[l-1] inside the box
+int effective_levels(const nyxrt_ctx *c) {
+    const double diag2 = (double)c->g.nx * c->g.nx + (double)c->g.ny * c->g.ny + (double)c->g.nz * c->g.nz;
+    int nlev = 1;
+    while (nlev <= c->p.level_max && c->r2_split[nlev - 1] < diag2) ++nlev;
+    return nlev;
+}
+
+uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, int staging) {
+    Bump b{static_cast<char *>(base), 0};
+    const long long n = max_sources > 0 ? max_sources : 1;
+    c->absorber = b.take<double>(c->ncell);
+    c->partial = b.take<double>(NPARTIAL);
+    c->scalars = b.take<double>(8);
+    c->ls = b.take<LoopState>(1);
+    c->ds = b.take<DevStats>(1);
+    long long total = 0;
+    for (int l = 0; l < MAXLEV; ++l) {
+        c->pool.off[l] = total;
+        c->pool.cap[l] = l < c->nlev ? (l == 0 ? 2 * B : 5 * B) : 0;
+        total += c->pool.cap[l];
+    }
+    c->pool.key = b.take<uint64_t>(total);
+    c->pool.s = b.take<double>(total);
+    c->pool.tau = b.take<double>(total);
+    c->pool.N = b.take<double>(total);
+    SrcBufs &s = c->sb;
+    s.pos = b.take<double>(3 * n);
+    s.L = b.take<double>(n);
+    s.key_a = b.take<long long>(n);
+    s.key_b = b.take<long long>(n);
+    s.idx_a = b.take<int>(n);
+    s.idx_b = b.take<int>(n);
+    s.flag = b.take<int>(n);
+    s.gid = b.take<int>(n);
+    s.par = b.take<int>(n);
+    s.lab_a = b.take<int>(n);
+    s.lab_b = b.take<int>(n);
+    s.bin_a = b.take<int>(n);
+    s.bin_b = b.take<int>(n);
+    for (int k = 0; k < 2; ++k) {
+        s.cell[k] = b.take<int4>(n);
+        s.L2[k] = b.take<double>(n);
+        s.r[k] = b.take<double>(n);
+        s.ckey[k] = b.take<long long>(n);
+    }
+    s.bad = b.take<int>(4);
+    s.dirs = b.take<double>(3ull * 12ull << (2 * c->p.samp_level));
+    s.cub_bytes = cub_temp_bytes(n);
+    s.cub_tmp = b.take<char>(s.cub_bytes);
+    if (staging) {
+        c->st_nH = b.take<char>(c->ncell * field_elem(c));
+        c->st_xHI = b.take<char>(c->ncell * field_elem(c));
+        c->st_gamma = b.take<double>(c->ncell);
+        c->st_heat = b.take<double>(c->ncell);
+    } else {
+        c->st_nH = c->st_xHI = nullptr;
+        c->st_gamma = c->st_heat = nullptr;
+    }
+    return ((b.off + 255) & ~uint64_t(255));
+}
+
+template <int GEOM>
+void launch_march(const MarchArgs &a, int blocks, cudaStream_t st) {
+    march_kernel<GEOM><<<blocks, MARCH_THREADS, 0, st>>>(a);
+}
+
+int geom_template(int mode) { return mode == 2 ? 3 : mode; }
+
+// ---- source pass: dedup + sort, optional radius + merge -------------------------------------------
+int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
+    SrcBufs &s = ctx->sb;
+    const long long n = ctx->n_src;
+    const GridDims gd{ctx->g.nx, ctx->g.ny, ctx->g.nz};
+    ctx->n_dedup = ctx->n_cat = 0;
+    ctx->cat_sel = 0;
+    if (n == 0) return NYXRT_OK;
+    int key_bits = 1;
+    while (((long long)1 << key_bits) < ctx->ncell) ++key_bits;
+    size_t tb = s.cub_bytes;
+    // (a1) stable sort by cell key, run heads, sequential flux sums
+    iota_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.idx_a, n);
+    CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.key_a, s.key_b, s.idx_a, s.idx_b, (int)n, 0, key_bits, st));
+    head_flags_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.key_b, n, s.flag);
+    tb = s.cub_bytes;
+    CU(cub::DeviceScan::InclusiveSum(s.cub_tmp, tb, s.flag, s.gid, (int)n, st));
+    dedup_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.key_b, s.idx_b, s.flag, s.gid, n, s.L, gd, s.cell[0], s.L2[0],
+                                                      s.ckey[0]);
+    int nd = 0;
+    CU(cudaMemcpyAsync(&nd, s.gid + (n - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    ctx->n_dedup = ctx->n_cat = nd;
+    fill_double_kernel<<<blocks_for(nd, 256), 256, 0, st>>>(s.r[0], nd, 0.0);
+    if (!do_merge) return NYXRT_OK;
+    // (a2) bubble radii
+    const int ndir = 12 << (2 * ctx->p.samp_level);
+    pix2dir_kernel<<<blocks_for(ndir, 128), 128, 0, st>>>(ctx->p.samp_level, 0, ndir, s.dirs);
+    const unsigned rb = blocks_for((long long)nd * 32, 256);
+    if (ctx->g.field_dtype)
+        radius_kernel<float><<<rb, 256, 0, st>>>(s.cell[0], nd, (const float *)ctx->d_xHI, gd, s.dirs, ndir,
+                                                  ctx->p.delta_r, ctx->p.r_max, ctx->p.x_th, ctx->p.f_req,
+                                                  ctx->p.n_min_samples, s.r[0]);
+    else
+        radius_kernel<double><<<rb, 256, 0, st>>>(s.cell[0], nd, (const double *)ctx->d_xHI, gd, s.dirs, ndir,
+                                                   ctx->p.delta_r, ctx->p.r_max, ctx->p.x_th, ctx->p.f_req,
+                                                   ctx->p.n_min_samples, s.r[0]);
+    // (a3) links between overlapping bubbles: bins of width W >= the largest link distance
+    const double X = 2.0 * ctx->p.f_ov * ctx->p.r_max;
+    long long Wl = (long long)floor(sqrt(X * X + ctx->p.eps)) + 1;
+    if (Wl < 1) Wl = 1;
+    if (Wl > (1 << 20)) Wl = 1 << 20;
+    const int W = (int)Wl;
+    const int nbx = (ctx->g.nx + W - 1) / W, nby = (ctx->g.ny + W - 1) / W, nbz = (ctx->g.nz + W - 1) / W;
+    int bin_bits = 1;
+    while (((long long)1 << bin_bits) < (long long)nbx * nby * nbz) ++bin_bits;
+    const unsigned nb = blocks_for(nd, 256);
+    bin_kernel<<<nb, 256, 0, st>>>(s.cell[0], nd, W, nbx, nby, s.bin_a, s.idx_a);
+    tb = s.cub_bytes;
+    CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.bin_a, s.bin_b, s.idx_a, s.idx_b, nd, 0, bin_bits, st));
+    iota_kernel<<<nb, 256, 0, st>>>(s.par, nd);
+    link_kernel<<<nb, 256, 0, st>>>(s.cell[0], s.r[0], nd, W, nbx, nby, nbz, s.bin_b, s.idx_b, ctx->p.f_ov, ctx->p.eps,
+                                    s.par);
+    // groups: label = smallest member; members in ascending catalogue order (stable sort by label)
+    label_kernel<<<nb, 256, 0, st>>>(s.par, nd, s.lab_a, s.idx_a);
+    int lab_bits = 1;
+    while (((long long)1 << lab_bits) < nd) ++lab_bits;
+    tb = s.cub_bytes;
+    CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.lab_a, s.lab_b, s.idx_a, s.idx_b, nd, 0, lab_bits, st));
+    head_flags_int_kernel<<<nb, 256, 0, st>>>(s.lab_b, nd, s.flag);
+    tb = s.cub_bytes;
+    CU(cub::DeviceScan::InclusiveSum(s.cub_tmp, tb, s.flag, s.gid, nd, st));
+    collapse_kernel<<<nb, 256, 0, st>>>(s.lab_b, s.idx_b, s.flag, s.gid, nd, s.cell[0], s.L2[0], s.r[0], gd, s.cell[1],
+                                        s.L2[1], s.r[1], s.ckey[1]);
+    int nm = 0;
+    CU(cudaMemcpyAsync(&nm, s.gid + (nd - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    // final sort by cell key; keys are unique
+    iota_kernel<<<blocks_for(nm, 256), 256, 0, st>>>(s.idx_a, nm);
+    tb = s.cub_bytes;
+    CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.ckey[1], s.ckey[0], s.idx_a, s.idx_b, nm, 0, key_bits, st));
+    gather_catalog_kernel<<<blocks_for(nm, 256), 256, 0, st>>>(s.idx_b, nm, s.cell[1], s.L2[1], s.r[1], s.cell[0],
+                                                                s.L2[0], s.r[0]);
+    ctx->n_cat = nm;
+    CU(cudaGetLastError());
+    return NYXRT_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+int nyxrt_version(void) { return 100; }
+int nyxrt_sizeof_grid(void) { return (int)sizeof(nyxrt_grid); }
+int nyxrt_sizeof_params(void) { return (int)sizeof(nyxrt_params); }
+int nyxrt_sizeof_stats(void) { return (int)sizeof(nyxrt_stats); }
+
+const char *nyxrt_last_error(const nyxrt_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+
+int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx **out) {
+    if (!grid || !params || !out) return NYXRT_EINVAL;
+    *out = nullptr;
+    const nyxrt_grid &g = *grid;
+    const nyxrt_params &p = *params;
+    if (g.nx < 1 || g.ny < 1 || g.nz < 1 || g.nx > (1 << 20) || g.ny > (1 << 20) || g.nz > (1 << 20)) return NYXRT_EINVAL;
+    if ((long long)g.nx * g.ny * g.nz >= ((long long)1 << 40)) return NYXRT_EINVAL;
+    if (g.field_dtype != 0 && g.field_dtype != 1) return NYXRT_EINVAL;
+    if (!(g.dx_cm > 0.0) || !(g.pos_unit_cm > 0.0) || g.periodic != 0) return NYXRT_EINVAL;
+    if (!(p.sigma_cm2 > 0.0) || !(p.n_min_ray > 0.0) || !(p.tau_max > 0.0)) return NYXRT_EINVAL;
+    if (p.level_max < 0 || p.level_max > 13 || p.geom_mode < 0 || p.geom_mode > 4) return NYXRT_EINVAL;
+    if (p.merge < 0 || p.merge > 2 || p.samp_level < 0 || p.samp_level > 8 || !(p.delta_r > 0.0)) return NYXRT_EINVAL;
+    if (!(p.r_max >= 0.0) || !(p.f_ov >= 0.0)) return NYXRT_EINVAL;
+    nyxrt_ctx *ctx = new (std::nothrow) nyxrt_ctx();
+    if (!ctx) return NYXRT_ENOMEM;
+    memset(ctx, 0, sizeof *ctx);
+    ctx->g = g;
+    ctx->p = p;
+    ctx->ncell = (long long)g.nx * g.ny * g.nz;
+    const double PI = 0x1.921fb54442d18p+1;
+    for (int l = 0; l < MAXLEV; ++l) {
+        ctx->r2_split[l] = std::ldexp(3.0 / (PI * p.n_min_ray), 2 * l);   // Eq. 4
+        ctx->K[l] = std::ldexp(std::sqrt(PI / 3.0), -l);                  // sqrt(4 pi / (12 4^l))
+    }
+    ctx->nlev = effective_levels(ctx);
+    cudaError_t e = cudaSetDevice(g.device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, g.device);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking);
+    for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev[k]);
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ls, sizeof(LoopState));
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ds, sizeof(DevStats));
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_scalars, 8 * sizeof(double));
+    int occ = 0;
+    if (e == cudaSuccess) {
+        switch (geom_template(p.geom_mode)) {
+            case 0: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<0>, MARCH_THREADS, 0); break;
+            case 1: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<1>, MARCH_THREADS, 0); break;
+            case 4: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<4>, MARCH_THREADS, 0); break;
+            default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<3>, MARCH_THREADS, 0); break;
+        }
+    }
+    if (e != cudaSuccess) {
+        // no CUDA device / wrong architecture: there is no fallback
+        nyxrt_destroy(ctx);
+        return NYXRT_ECUDA;
+    }
+    ctx->sm_count = prop.multiProcessorCount;
+    ctx->march_blocks = ctx->sm_count * (occ > 0 ? occ : 1);
+    *out = ctx;
+    return NYXRT_OK;
+}
+
+void nyxrt_destroy(nyxrt_ctx *ctx) {
+    if (!ctx) return;
+    for (int k = 0; k < 4; ++k)
+        if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    if (ctx->h_ls) cudaFreeHost(ctx->h_ls);
+    if (ctx->h_ds) cudaFreeHost(ctx->h_ds);
+    if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
+    delete ctx;
+}
+
+int nyxrt_workspace_bytes(const nyxrt_ctx *cctx, int64_t max_sources, int64_t batch_rays, int32_t host_staging,
+                          uint64_t *bytes) {
+    nyxrt_ctx *ctx = const_cast<nyxrt_ctx *>(cctx);
+    if (!ctx || !bytes || max_sources < 0 || batch_rays < 0 || max_sources >= (1ll << 30))
+        return fail(ctx, NYXRT_EINVAL, "workspace_bytes: bad argument");
+    if (ctx->ws) return fail(ctx, NYXRT_ESTATE, "workspace_bytes: query before set_workspace");
+    const long long B = batch_rays ? batch_rays : (1ll << 21);
+    if (B < 32) return fail(ctx, NYXRT_EINVAL, "workspace_bytes: batch_rays must be >= 32");
+    *bytes = layout(ctx, nullptr, max_sources, B, host_staging);
+    return NYXRT_OK;
+}
+
+int nyxrt_set_workspace(nyxrt_ctx *ctx, void *d_ws, uint64_t bytes, int64_t max_sources, int64_t batch_rays,
+                        int32_t host_staging) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!d_ws || ((uintptr_t)d_ws & 255) || max_sources < 0 || batch_rays < 0 || max_sources >= (1ll << 30))
+        return fail(ctx, NYXRT_EINVAL, "set_workspace: bad argument (pointer must be 256-byte aligned)");
+    const long long B = batch_rays ? batch_rays : (1ll << 21);
+    if (B < 32) return fail(ctx, NYXRT_EINVAL, "set_workspace: batch_rays must be >= 32");
+    ctx->ws = nullptr;
+    const uint64_t need = layout(ctx, nullptr, max_sources, B, host_staging);
+    if (bytes < need) return fail(ctx, NYXRT_ENOMEM, "set_workspace: %llu bytes given, %llu needed",
+                                  (unsigned long long)bytes, (unsigned long long)need);
+    layout(ctx, d_ws, max_sources, B, host_staging);
+    ctx->ws = d_ws;
+    ctx->ws_bytes = bytes;
+    ctx->max_sources = max_sources;
+    ctx->batch_rays = B;
+    ctx->host_staging = host_staging;
+    ctx->have_fields = ctx->have_sources = ctx->have_catalog = false;
+    return NYXRT_OK;
+}
+
+int nyxrt_set_fields(nyxrt_ctx *ctx, const void *d_nH, const void *d_xHI, void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!d_nH || !d_xHI) return fail(ctx, NYXRT_EINVAL, "set_fields: null field pointer");
+    if (!ctx->ws) return fail(ctx, NYXRT_ESTATE, "set_fields: no workspace");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->g.device));
+    const int use_flag = ctx->p.geom_mode == 3;
+    if (ctx->g.field_dtype)
+        prep_fields_kernel<float><<<NPARTIAL, 256, 0, st>>>((const float *)d_nH, (const float *)d_xHI, ctx->absorber,
+                                                            ctx->ncell, ctx->p.n_th, use_flag, ctx->partial);
+    else
+        prep_fields_kernel<double><<<NPARTIAL, 256, 0, st>>>((const double *)d_nH, (const double *)d_xHI, ctx->absorber,
+                                                             ctx->ncell, ctx->p.n_th, use_flag, ctx->partial);
+    sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 0);
+    CU(cudaGetLastError());
+    ctx->d_nH = d_nH;
+    ctx->d_xHI = d_xHI;
+    ctx->have_fields = true;
+    return NYXRT_OK;
+}
+
+int nyxrt_set_sources(nyxrt_ctx *ctx, int64_t n, const double *pos, const double *L, void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    ctx->have_sources = false;
+    ctx->have_catalog = false;
+    if (n < 0 || (n > 0 && (!pos || !L))) return fail(ctx, NYXRT_EINVAL, "set_sources: bad argument");
+    if (!ctx->ws) return fail(ctx, NYXRT_ESTATE, "set_sources: no workspace");
+    if (n > ctx->max_sources) return fail(ctx, NYXRT_ENOMEM, "set_sources: %lld sources, workspace sized for %lld",
+                                          (long long)n, ctx->max_sources);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->g.device));
+    ctx->n_src = n;
+    if (n > 0) {
+        SrcBufs &s = ctx->sb;
+        CU(cudaMemcpyAsync(s.pos, pos, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(s.L, L, n * sizeof(double), cudaMemcpyHostToDevice, st));
+        CU(cudaMemsetAsync(s.bad, 0, sizeof(int), st));
+        const GridDims gd{ctx->g.nx, ctx->g.ny, ctx->g.nz};
+        snap_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.pos, s.L, n, gd, ctx->g.box_lo[0], ctx->g.box_lo[1],
+                                                         ctx->g.box_lo[2], ctx->g.pos_unit_cm, ctx->g.dx_cm, s.key_a,
+                                                         s.bad);
+        int bad = 0;
+        CU(cudaMemcpyAsync(&bad, s.bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (bad) {
+            ctx->n_src = 0;
+            return fail(ctx, NYXRT_EINVAL, "set_sources: a source lies outside the box or has an invalid luminosity");
+        }
+    }
+    ctx->have_sources = true;
+    return NYXRT_OK;
+}
+
+int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs, void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!d_gamma) return fail(ctx, NYXRT_EINVAL, "trace: null output");
+    if (!ctx->ws || !ctx->have_fields || !ctx->have_sources)
+        return fail(ctx, NYXRT_ESTATE, "trace: workspace, fields and sources must be set first");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->g.device));
+    CU(cudaEventRecord(ctx->ev[0], st));
+    // ---- sources ----
+    bool do_merge = ctx->p.merge == 1;
+    if (ctx->p.merge == 2) {
+        CU(cudaMemcpyAsync(ctx->h_scalars, ctx->scalars, sizeof(double), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        do_merge = ctx->h_scalars[0] / (double)ctx->ncell > ctx->p.automerge_xmean;
+    }
+    // the snap keys are consumed by the sort; keep them for a later trace by sorting out of place
+    int rc = source_pass(ctx, st, do_merge);
+    if (rc) return rc;
+    ctx->have_catalog = true;
+    const SrcBufs &s = ctx->sb;
+    sum_flux_kernel<<<1, 256, 0, st>>>(s.L2[0], ctx->n_cat, ctx->scalars + 2);
+    CU(cudaEventRecord(ctx->ev[1], st));
+    // ---- ray loop ----
+    CU(cudaMemsetAsync(d_gamma, 0, ctx->ncell * sizeof(double), st));
+    CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
+    memset(ctx->h_ls, 0, sizeof(LoopState));
+    ctx->h_ls->n_cat = ctx->n_cat;
+    ctx->h_ls->batch_rays = ctx->batch_rays;
+    CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
+    MarchArgs a;
+    memset(&a, 0, sizeof a);
+    a.absorber = ctx->absorber;
+    a.acc = d_gamma;
+    a.cat_cell = s.cell[0];
+    a.cat_L = s.L2[0];
+    a.pool = ctx->pool;
+    a.ls = ctx->ls;
+    a.ds = ctx->ds;
+    a.nx = ctx->g.nx; a.ny = ctx->g.ny; a.nz = ctx->g.nz;
+    a.level_max = ctx->p.level_max;
+    a.sdx = ctx->p.sigma_cm2 * ctx->g.dx_cm;
+    a.tau_max = ctx->p.tau_max;
+    for (int l = 0; l < MAXLEV; ++l) { a.r2_split[l] = ctx->r2_split[l]; a.K[l] = ctx->K[l]; }
+    const int gt = geom_template(ctx->p.geom_mode);
+    const int emit_blocks = ctx->sm_count * 4;
+    int chunk = 8;
+    for (;;) {
+        for (int i = 0; i < chunk; ++i) {
+            sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev);
+            emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0]);
+            switch (gt) {
+                case 0: launch_march<0>(a, ctx->march_blocks, st); break;
+                case 1: launch_march<1>(a, ctx->march_blocks, st); break;
+                case 4: launch_march<4>(a, ctx->march_blocks, st); break;
+                default: launch_march<3>(a, ctx->march_blocks, st); break;
+            }
+        }
+        CU(cudaMemcpyAsync(ctx->h_ls, ctx->ls, sizeof(LoopState), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        if (ctx->h_ls->overflow) return fail(ctx, NYXRT_EOVERFLOW, "trace: ray pool overflow at level %d", ctx->h_ls->level + 1);
+        if (ctx->h_ls->done) break;
+        if (chunk < 256) chunk *= 2;
+    }
+    CU(cudaEventRecord(ctx->ev[2], st));
+    // ---- finalise ----
+    const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
+    finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->absorber, ctx->ncell, V, ctx->p.e_excess_erg,
+                                              ctx->partial);
+    sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
+    CU(cudaEventRecord(ctx->ev[3], st));
+    CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(ctx->h_scalars, ctx->scalars, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if (hs) {
+        memset(hs, 0, sizeof *hs);
+        const DevStats &d = *ctx->h_ds;
+        for (int l = 0; l < MAXLEV; ++l) {
+            hs->spawned[l] = d.spawned[l]; hs->split[l] = d.split[l]; hs->killed_tau[l] = d.killed_tau[l];
+            hs->exited[l] = d.exited[l]; hs->killed_lmax[l] = d.killed_lmax[l];
+        }
+        hs->segments = d.segments;
+        hs->zero_len_segments = d.zero_len;
+        hs->n_src_in = (uint64_t)ctx->n_src;
+        hs->n_src_dedup = (uint64_t)ctx->n_dedup;
+        hs->n_src_merged = (uint64_t)ctx->n_cat;
+        hs->iterations = ctx->h_ls->iterations;
+        hs->peak_pool_rays = ctx->h_ls->peak_pool;
+        hs->photons_emitted = ctx->n_cat ? ctx->h_scalars[2] : 0.0;
+        hs->photons_absorbed = ctx->h_scalars[1];
+        hs->photons_escaped = d.escaped;
+        hs->photons_residual = d.residual;
+        hs->photons_lost = d.lost;
+        cudaEventElapsedTime(&hs->ms_sources, ctx->ev[0], ctx->ev[1]);
+        cudaEventElapsedTime(&hs->ms_loop, ctx->ev[1], ctx->ev[2]);
+        cudaEventElapsedTime(&hs->ms_finalise, ctx->ev[2], ctx->ev[3]);
+        cudaEventElapsedTime(&hs->ms_total, ctx->ev[0], ctx->ev[3]);
+    }
+    return NYXRT_OK;
+}
+
+int nyxrt_get_catalog(nyxrt_ctx *ctx, int64_t cap, int32_t *cell_ijk, double *L, double *radius, int64_t *n_out) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!n_out || cap < 0) return fail(ctx, NYXRT_EINVAL, "get_catalog: bad argument");
+    if (!ctx->have_catalog) return fail(ctx, NYXRT_ESTATE, "get_catalog: no trace has run");
+    CU(cudaSetDevice(ctx->g.device));
+    *n_out = ctx->n_cat;
+    const long long m = cap < ctx->n_cat ? cap : ctx->n_cat;
+    if (m == 0) return NYXRT_OK;
+    const SrcBufs &s = ctx->sb;
+    if (cell_ijk) {
+        int4 *tmp = new (std::nothrow) int4[m];
+        if (!tmp) return fail(ctx, NYXRT_ENOMEM, "get_catalog: host allocation failed");
+        cudaError_t e = cudaMemcpy(tmp, s.cell[0], m * sizeof(int4), cudaMemcpyDeviceToHost);
+        for (long long a = 0; a < m && e == cudaSuccess; ++a) {
+            cell_ijk[3 * a] = tmp[a].x; cell_ijk[3 * a + 1] = tmp[a].y; cell_ijk[3 * a + 2] = tmp[a].z;
+        }
+        delete[] tmp;
+        CU(e);
+    }
+    if (L) CU(cudaMemcpy(L, s.L2[0], m * sizeof(double), cudaMemcpyDeviceToHost));
+    if (radius) CU(cudaMemcpy(radius, s.r[0], m * sizeof(double), cudaMemcpyDeviceToHost));
+    return NYXRT_OK;
+}
+
+int nyxrt_step_host(nyxrt_ctx *ctx, const void *h_nH, const void *h_xHI, int64_t n_src, const double *pos,
+                    const double *L, double *h_gamma, double *h_heat, nyxrt_stats *hs) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!h_nH || !h_xHI || !h_gamma) return fail(ctx, NYXRT_EINVAL, "step_host: null pointer");
+    if (!ctx->ws || !ctx->host_staging) return fail(ctx, NYXRT_ESTATE, "step_host: workspace lacks host staging");
+    cudaStream_t st = ctx->own_stream;
+    CU(cudaSetDevice(ctx->g.device));
+    const size_t fb = (size_t)ctx->ncell * field_elem(ctx);
+    CU(cudaMemcpyAsync(ctx->st_nH, h_nH, fb, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(ctx->st_xHI, h_xHI, fb, cudaMemcpyHostToDevice, st));
+    int rc = nyxrt_set_fields(ctx, ctx->st_nH, ctx->st_xHI, st);
+    if (rc) return rc;
+    rc = nyxrt_set_sources(ctx, n_src, pos, L, st);
+    if (rc) return rc;
+    rc = nyxrt_trace(ctx, ctx->st_gamma, h_heat ? ctx->st_heat : nullptr, hs, st);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(h_gamma, ctx->st_gamma, ctx->ncell * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (h_heat) CU(cudaMemcpyAsync(h_heat, ctx->st_heat, ctx->ncell * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return NYXRT_OK;
+}
+
+int nyxrt_pix2dir(nyxrt_ctx *ctx, int32_t level, int64_t pix_begin, int64_t n, double *dir_xyz) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (level < 0 || level > 14 || pix_begin < 0 || n < 0 || !dir_xyz || pix_begin + n > (12ll << (2 * level)))
+        return fail(ctx, NYXRT_EINVAL, "pix2dir: bad argument");
+    if (n == 0) return NYXRT_OK;
+    CU(cudaSetDevice(ctx->g.device));
+    double *d = nullptr;
+    CU(cudaMalloc(&d, 3 * n * sizeof(double)));
+    pix2dir_kernel<<<blocks_for(n, 128), 128>>>(level, pix_begin, n, d);
+    cudaError_t e = cudaMemcpy(dir_xyz, d, 3 * n * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    CU(e);
+    return NYXRT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,273 @@
+// The source pass on the device (rows a1-a3): snap + dedup + sort, MAX_RADIUS and
+// MERGE_SOURCES of Alg. 3 (text 313-333).  The paper runs this on the host I/O rank
+// over all pairs; here the pair search is binned by cell and the union-find is lock-free, which gives
+// the same connected components.  Sums that later steer rounding (dedup flux, centroid) are sequential
+// in catalogue order, as DESIGN.md's DEC list requires.
+#pragma once
+#include <stdint.h>
+
+#include "healpix.cuh"
+
+namespace nyxrt {
+
+struct GridDims { int nx, ny, nz; };
+
+// key = linear cell index, or -1 and *bad = 1 if the source is outside the box / L invalid (reading R2)
+__global__ void snap_kernel(const double *__restrict__ pos, const double *__restrict__ L, long long n, GridDims g,
+                            double lo0, double lo1, double lo2, double unit, double dx,
+                            long long *__restrict__ key, int *bad) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    const double u0 = (pos[3 * a] - lo0) * unit / dx, u1 = (pos[3 * a + 1] - lo1) * unit / dx,
+                 u2 = (pos[3 * a + 2] - lo2) * unit / dx;
+    const double l = L[a];
+    bool ok = (l >= 0.0) && !isinf(l);
+    ok = ok && (u0 >= 0.0) && (u0 < (double)g.nx) && (u1 >= 0.0) && (u1 < (double)g.ny) && (u2 >= 0.0) &&
+         (u2 < (double)g.nz);
+    long long k = -1;
+    if (ok) {
+        const long long i = (long long)floor(u0), j = (long long)floor(u1), kk = (long long)floor(u2);
+        k = (kk * g.ny + j) * g.nx + i;
+    } else {
+        *bad = 1;
+    }
+    key[a] = k;
+}
+
+__global__ void head_flags_kernel(const long long *__restrict__ key, long long n, int *__restrict__ flag) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    flag[t] = (t == 0 || key[t] != key[t - 1]) ? 1 : 0;
+}
+
+// one thread per run of equal keys: flux summed in input order (the sort is stable)
+__global__ void dedup_kernel(const long long *__restrict__ key, const int *__restrict__ idx,
+                             const int *__restrict__ flag, const int *__restrict__ gid_incl, long long n,
+                             const double *__restrict__ L, GridDims g, int4 *__restrict__ out_cell,
+                             double *__restrict__ out_L, long long *__restrict__ out_key) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n || !flag[t]) return;
+    const long long k = key[t];
+    double sum = 0.0;
+    for (long long u = t; u < n && key[u] == k; ++u) sum = sum + L[idx[u]];
+    const int gid = gid_incl[t] - 1;
+    const int i = (int)(k % g.nx), j = (int)((k / g.nx) % g.ny), kk = (int)(k / ((long long)g.nx * g.ny));
+    out_cell[gid] = make_int4(i, j, kk, 0);
+    out_L[gid] = sum;
+    out_key[gid] = k;
+}
+
+template <typename T>
+__device__ __forceinline__ double ion_frac(const T *xHI, long long c) { return 1.0 - (double)xHI[c]; }
+
+// MAX_RADIUS: one warp per source, lanes share the 12*4^samp_level directions of a shell.
+template <typename T>
+__global__ void radius_kernel(const int4 *__restrict__ cell, long long n, const T *__restrict__ xHI, GridDims g,
+                              const double *__restrict__ dirs, int ndir, double delta_r, double r_max, double x_th,
+                              double f_req, int n_min_samples, double *__restrict__ r_out) {
+    const long long a = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (a >= n) return;
+    const int4 c = cell[a];
+    const double x0 = ion_frac(xHI, ((long long)c.z * g.ny + c.y) * g.nx + c.x);
+    if (x0 < x_th) { if (lane == 0) r_out[a] = 0.0; return; }
+    double r = delta_r, res = -1.0;
+    while (r <= r_max) {
+        int ntot = 0, nion = 0;
+        for (int q = lane; q < ndir; q += 32) {
+            const long long i = c.x + (long long)floor(fma(r, dirs[3 * q], 0.5));
+            const long long j = c.y + (long long)floor(fma(r, dirs[3 * q + 1], 0.5));
+            const long long k = c.z + (long long)floor(fma(r, dirs[3 * q + 2], 0.5));
+            if (i < 0 || i >= g.nx || j < 0 || j >= g.ny || k < 0 || k >= g.nz) continue;
+            ++ntot;
+            if (ion_frac(xHI, (k * g.ny + j) * g.nx + i) >= x_th) ++nion;
+        }
+        ntot = __reduce_add_sync(0xffffffffu, ntot);
+        nion = __reduce_add_sync(0xffffffffu, nion);
+        bool pass;
+        if (ntot == 0) pass = false;
+        else if (ntot < n_min_samples) pass = (nion == ntot);
+        else pass = ((double)nion >= f_req * (double)ntot);
+        if (!pass) { res = r - delta_r; break; }
+        r = r + delta_r;
+    }
+    if (lane == 0) r_out[a] = (res >= 0.0) ? res : r_max;
+}
+
+// ---- union-find, smaller index wins (so the root of a component is its smallest member) -------------
+// par[x] <= x always, so following parents strictly descends until a root (par[r] == r).  Reads bypass
+// L1 (volatile): other threads hook roots concurrently with atomicCAS.  Path compression only rewrites
+// non-roots with one of their ancestors, hooking only rewrites roots, so the two never collide.
+__device__ __forceinline__ int uf_find(int *par, int a) {
+    volatile int *vp = par;
+    int curr = vp[a];
+    if (curr != a) {
+        int prev = a, next;
+        while (curr > (next = vp[curr])) {
+            vp[prev] = next;
+            prev = curr;
+            curr = next;
+        }
+    }
+    return curr;
+}
+
+__device__ __forceinline__ void uf_unite(int *par, int a, int b) {
+    for (;;) {
+        a = uf_find(par, a);
+        b = uf_find(par, b);
+        if (a == b) return;
+        if (a > b) { const int t = a; a = b; b = t; }
+        // hook the larger root b under the smaller root a
+        const int old = atomicCAS(par + b, b, a);
+        if (old == b) return;
+    }
+}
+
+__global__ void iota_kernel(int *p, long long n) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a < n) p[a] = (int)a;
+}
+
+__global__ void bin_kernel(const int4 *__restrict__ cell, long long n, int W, int nbx, int nby,
+                           int *__restrict__ bin, int *__restrict__ idx) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    const int4 c = cell[a];
+    bin[a] = ((c.z / W) * nby + (c.y / W)) * nbx + (c.x / W);
+    idx[a] = (int)a;
+}
+
+__device__ __forceinline__ long long lower_bound_int(const int *v, long long n, int x) {
+    long long lo = 0, hi = n;
+    while (lo < hi) {
+        const long long mid = (lo + hi) >> 1;
+        if (v[mid] < x) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+// link test of Alg. 3 (PAPER.md:367-370 with the text's epsilon, 331): integer d^2, fp64 right-hand side
+__global__ void link_kernel(const int4 *__restrict__ cell, const double *__restrict__ rad, long long n, int W,
+                            int nbx, int nby, int nbz, const int *__restrict__ sbin, const int *__restrict__ sidx,
+                            double f_ov, double eps, int *par) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    const double ra = rad[a];
+    if (!(ra > 0.0)) return;
+    const int4 ca = cell[a];
+    const int bx = ca.x / W, by = ca.y / W, bz = ca.z / W;
+    for (int dz = -1; dz <= 1; ++dz)
+        for (int dy = -1; dy <= 1; ++dy)
+            for (int dx = -1; dx <= 1; ++dx) {
+                const int x = bx + dx, y = by + dy, z = bz + dz;
+                if (x < 0 || x >= nbx || y < 0 || y >= nby || z < 0 || z >= nbz) continue;
+                const int b = (z * nby + y) * nbx + x;
+                for (long long t = lower_bound_int(sbin, n, b); t < n && sbin[t] == b; ++t) {
+                    const int o = sidx[t];
+                    if (o <= a) continue;                                   // each pair once (a < b)
+                    const double rb = rad[o];
+                    if (!(rb > 0.0)) continue;
+                    const int4 cb = cell[o];
+                    const long long ex = (long long)ca.x - cb.x, ey = (long long)ca.y - cb.y, ez = (long long)ca.z - cb.z;
+                    const long long d2 = ex * ex + ey * ey + ez * ez;
+                    const double rs = f_ov * (ra + rb);
+                    if ((double)d2 <= rs * rs + eps) uf_unite(par, (int)a, o);
+                }
+            }
+}
+
+__global__ void label_kernel(int *par, long long n, int *__restrict__ label, int *__restrict__ idx) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    label[a] = uf_find(par, (int)a);
+    idx[a] = (int)a;
+}
+
+__global__ void head_flags_int_kernel(const int *__restrict__ key, long long n, int *__restrict__ flag) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    flag[t] = (t == 0 || key[t] != key[t - 1]) ? 1 : 0;
+}
+
+// one thread per group (members = a run of equal labels, ascending catalogue index): flux sum, max
+// radius, flux-weighted centroid, round, snap to the nearest member (first on ties) -- PAPER.md:378-387
+__global__ void collapse_kernel(const int *__restrict__ slabel, const int *__restrict__ sidx,
+                                const int *__restrict__ flag, const int *__restrict__ gid_incl, long long n,
+                                const int4 *__restrict__ cell, const double *__restrict__ L,
+                                const double *__restrict__ rad, GridDims g, int4 *__restrict__ out_cell,
+                                double *__restrict__ out_L, double *__restrict__ out_r,
+                                long long *__restrict__ out_key) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n || !flag[t]) return;
+    const int lab = slabel[t];
+    long long e = t;
+    double F = 0.0, R = 0.0, n0 = 0.0, n1 = 0.0, n2 = 0.0;
+    for (; e < n && slabel[e] == lab; ++e) {
+        const int b = sidx[e];
+        const double l = L[b];
+        const int4 c = cell[b];
+        F = F + l;
+        if (rad[b] > R) R = rad[b];
+        n0 = n0 + l * (double)c.x;
+        n1 = n1 + l * (double)c.y;
+        n2 = n2 + l * (double)c.z;
+    }
+    int4 oc;
+    double oL, oR;
+    if (e - t == 1) {
+        const int b = sidx[t];
+        oc = cell[b]; oL = L[b]; oR = rad[b];
+    } else {
+        const long long r0 = (long long)floor(n0 / F + 0.5), r1 = (long long)floor(n1 / F + 0.5),
+                        r2 = (long long)floor(n2 / F + 0.5);
+        long long bestd = -1;
+        int best = -1;
+        for (long long u = t; u < e; ++u) {
+            const int4 c = cell[sidx[u]];
+            const long long ex = c.x - r0, ey = c.y - r1, ez = c.z - r2;
+            const long long d2 = ex * ex + ey * ey + ez * ez;
+            if (best < 0 || d2 < bestd) { best = sidx[u]; bestd = d2; }
+        }
+        oc = cell[best]; oL = F; oR = R;
+    }
+    const int gid = gid_incl[t] - 1;
+    out_cell[gid] = oc;
+    out_L[gid] = oL;
+    out_r[gid] = oR;
+    out_key[gid] = ((long long)oc.z * g.ny + oc.y) * g.nx + oc.x;
+}
+
+// gather a catalogue through a permutation (after the final sort by cell key)
+__global__ void gather_catalog_kernel(const int *__restrict__ perm, long long n, const int4 *__restrict__ cell,
+                                      const double *__restrict__ L, const double *__restrict__ rad,
+                                      int4 *__restrict__ out_cell, double *__restrict__ out_L,
+                                      double *__restrict__ out_r) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= n) return;
+    const int p = perm[a];
+    out_cell[a] = cell[p];
+    out_L[a] = L[p];
+    out_r[a] = rad ? rad[p] : 0.0;
+}
+
+__global__ void fill_double_kernel(double *p, long long n, double v) {
+    const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a < n) p[a] = v;
+}
+
+// sum of catalogue fluxes = photons emitted (fixed order: single block, strided then tree)
+__global__ void sum_flux_kernel(const double *__restrict__ L, long long n, double *out) {
+    __shared__ double sh[256];
+    double acc = 0.0;
+    for (long long i = threadIdx.x; i < n; i += blockDim.x) acc += L[i];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = blockDim.x >> 1; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = sh[0];
+}
+
+}  // namespace nyxrt

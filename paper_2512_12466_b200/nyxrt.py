@@ -1,0 +1,257 @@
+"""ctypes binding of include/nyxrt.h.  Same names as the C ABI; argument marshalling only.
+
+torch is used for what the task assigns to it: device memory (workspace, fields, outputs) and streams.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+MAXLEV = 16
+OK, EINVAL, ESTATE, ENOMEM, ECUDA, EOVERFLOW = 0, -1, -2, -3, -4, -5
+_ERRNAME = {EINVAL: "NYXRT_EINVAL", ESTATE: "NYXRT_ESTATE", ENOMEM: "NYXRT_ENOMEM", ECUDA: "NYXRT_ECUDA",
+            EOVERFLOW: "NYXRT_EOVERFLOW"}
+
+
+class NyxrtError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("%s (%d): %s" % (_ERRNAME.get(code, "?"), code, msg))
+        self.code = code
+
+
+class nyxrt_grid(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("field_dtype", C.c_int32),
+                ("dx_cm", C.c_double), ("box_lo", C.c_double * 3), ("pos_unit_cm", C.c_double),
+                ("periodic", C.c_int32), ("device", C.c_int32)]
+
+
+class nyxrt_params(C.Structure):
+    _fields_ = [("sigma_cm2", C.c_double), ("n_min_ray", C.c_double), ("tau_max", C.c_double),
+                ("n_th", C.c_double), ("e_excess_erg", C.c_double), ("automerge_xmean", C.c_double),
+                ("delta_r", C.c_double), ("r_max", C.c_double), ("f_ov", C.c_double), ("x_th", C.c_double),
+                ("f_req", C.c_double), ("eps", C.c_double),
+                ("level_max", C.c_int32), ("geom_mode", C.c_int32), ("merge", C.c_int32),
+                ("n_min_samples", C.c_int32), ("samp_level", C.c_int32), ("reserved", C.c_int32)]
+
+
+class nyxrt_stats(C.Structure):
+    _fields_ = [("spawned", C.c_uint64 * MAXLEV), ("split", C.c_uint64 * MAXLEV),
+                ("killed_tau", C.c_uint64 * MAXLEV), ("exited", C.c_uint64 * MAXLEV),
+                ("killed_lmax", C.c_uint64 * MAXLEV),
+                ("segments", C.c_uint64), ("zero_len_segments", C.c_uint64),
+                ("n_src_in", C.c_uint64), ("n_src_dedup", C.c_uint64), ("n_src_merged", C.c_uint64),
+                ("iterations", C.c_uint64), ("peak_pool_rays", C.c_uint64),
+                ("photons_emitted", C.c_double), ("photons_absorbed", C.c_double),
+                ("photons_escaped", C.c_double), ("photons_residual", C.c_double), ("photons_lost", C.c_double),
+                ("ms_sources", C.c_float), ("ms_loop", C.c_float), ("ms_finalise", C.c_float),
+                ("ms_total", C.c_float)]
+
+    def as_dict(self):
+        d = {}
+        for name, _ in self._fields_:
+            v = getattr(self, name)
+            d[name] = list(v) if hasattr(v, "__len__") else v
+        return d
+
+
+EXPORTS = ["nyxrt_create", "nyxrt_workspace_bytes", "nyxrt_set_workspace", "nyxrt_set_fields", "nyxrt_set_sources",
+           "nyxrt_trace", "nyxrt_get_catalog", "nyxrt_step_host", "nyxrt_pix2dir", "nyxrt_last_error",
+           "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats"]
+
+_lib = None
+
+
+def lib():
+    """Loads libnyxrt.so; raises (never falls back) when it is missing."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path):
+            raise ImportError("libnyxrt.so is not built: run `python -m paper_2512_12466_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(path)
+        for name in EXPORTS:
+            getattr(L, name)
+        L.nyxrt_last_error.restype = C.c_char_p
+        L.nyxrt_last_error.argtypes = [C.c_void_p]
+        L.nyxrt_destroy.restype = None
+        L.nyxrt_destroy.argtypes = [C.c_void_p]
+        assert L.nyxrt_sizeof_grid() == C.sizeof(nyxrt_grid)
+        assert L.nyxrt_sizeof_params() == C.sizeof(nyxrt_params)
+        assert L.nyxrt_sizeof_stats() == C.sizeof(nyxrt_stats)
+        _lib = L
+    return _lib
+
+
+def _check(ctx, rc):
+    if rc != OK:
+        msg = lib().nyxrt_last_error(ctx).decode() if ctx else "no context"
+        raise NyxrtError(rc, msg)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+# ---- the C ABI, one Python function per entry point ---------------------------------------------------
+
+def nyxrt_create(grid, params):
+    ctx = C.c_void_p()
+    rc = lib().nyxrt_create(C.byref(grid), C.byref(params), C.byref(ctx))
+    if rc != OK:
+        raise NyxrtError(rc, "nyxrt_create failed (no CUDA device, or bad grid/params)")
+    return ctx
+
+
+def nyxrt_workspace_bytes(ctx, max_sources, batch_rays=0, host_staging=False):
+    n = C.c_uint64(0)
+    _check(ctx, lib().nyxrt_workspace_bytes(ctx, C.c_int64(max_sources), C.c_int64(batch_rays),
+                                            C.c_int32(1 if host_staging else 0), C.byref(n)))
+    return n.value
+
+
+def nyxrt_set_workspace(ctx, workspace, max_sources, batch_rays=0, host_staging=False):
+    assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()
+    _check(ctx, lib().nyxrt_set_workspace(ctx, C.c_void_p(workspace.data_ptr()), C.c_uint64(workspace.numel()),
+                                          C.c_int64(max_sources), C.c_int64(batch_rays),
+                                          C.c_int32(1 if host_staging else 0)))
+
+
+def nyxrt_set_fields(ctx, nH, xHI, stream=None):
+    assert nH.is_cuda and xHI.is_cuda and nH.is_contiguous() and xHI.is_contiguous() and nH.dtype == xHI.dtype
+    _check(ctx, lib().nyxrt_set_fields(ctx, C.c_void_p(nH.data_ptr()), C.c_void_p(xHI.data_ptr()), _stream_ptr(stream)))
+
+
+def nyxrt_set_sources(ctx, pos, L, stream=None):
+    pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+    L = np.ascontiguousarray(L, dtype=np.float64).reshape(-1)
+    assert len(pos) == len(L)
+    _check(ctx, lib().nyxrt_set_sources(ctx, C.c_int64(len(L)), pos.ctypes.data_as(C.c_void_p),
+                                        L.ctypes.data_as(C.c_void_p), _stream_ptr(stream)))
+
+
+def nyxrt_trace(ctx, gamma, heat=None, stream=None):
+    assert gamma.is_cuda and gamma.dtype == torch.float64 and gamma.is_contiguous()
+    assert heat is None or (heat.is_cuda and heat.dtype == torch.float64 and heat.is_contiguous())
+    st = nyxrt_stats()
+    _check(ctx, lib().nyxrt_trace(ctx, C.c_void_p(gamma.data_ptr()),
+                                  C.c_void_p(heat.data_ptr()) if heat is not None else None,
+                                  C.byref(st), _stream_ptr(stream)))
+    return st
+
+
+def nyxrt_get_catalog(ctx):
+    n = C.c_int64(0)
+    _check(ctx, lib().nyxrt_get_catalog(ctx, C.c_int64(0), None, None, None, C.byref(n)))
+    m = n.value
+    cell = np.zeros((m, 3), np.int32)
+    L = np.zeros(m)
+    r = np.zeros(m)
+    if m:
+        _check(ctx, lib().nyxrt_get_catalog(ctx, C.c_int64(m), cell.ctypes.data_as(C.c_void_p),
+                                            L.ctypes.data_as(C.c_void_p), r.ctypes.data_as(C.c_void_p), C.byref(n)))
+    return cell, L, r
+
+
+def nyxrt_step_host(ctx, nH, xHI, pos, L, gamma, heat=None):
+    """Host buffers in, host buffers out (torch CPU tensors or numpy arrays; pinned memory is fastest)."""
+    def hp(a):
+        return C.c_void_p(a.data_ptr()) if isinstance(a, torch.Tensor) else a.ctypes.data_as(C.c_void_p)
+    pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+    L = np.ascontiguousarray(L, dtype=np.float64).reshape(-1)
+    st = nyxrt_stats()
+    _check(ctx, lib().nyxrt_step_host(ctx, hp(nH), hp(xHI), C.c_int64(len(L)), pos.ctypes.data_as(C.c_void_p),
+                                      L.ctypes.data_as(C.c_void_p), hp(gamma), hp(heat) if heat is not None else None,
+                                      C.byref(st)))
+    return st
+
+
+def nyxrt_pix2dir(ctx, level, pix_begin, n):
+    out = np.zeros((n, 3))
+    _check(ctx, lib().nyxrt_pix2dir(ctx, C.c_int32(level), C.c_int64(pix_begin), C.c_int64(n),
+                                    out.ctypes.data_as(C.c_void_p)))
+    return out
+
+
+def nyxrt_destroy(ctx):
+    lib().nyxrt_destroy(ctx)
+
+
+# ---- small convenience wrapper used by tests / bench (still marshalling only) --------------------------
+
+def make_grid(shape_zyx, dx_cm, field_dtype=torch.float64, box_lo=(0.0, 0.0, 0.0), pos_unit_cm=None, device=0):
+    g = nyxrt_grid()
+    g.nz, g.ny, g.nx = [int(v) for v in shape_zyx]
+    g.field_dtype = 1 if field_dtype == torch.float32 else 0
+    g.dx_cm = float(dx_cm)
+    g.box_lo[:] = [float(v) for v in box_lo]
+    g.pos_unit_cm = float(dx_cm if pos_unit_cm is None else pos_unit_cm)
+    g.periodic = 0
+    g.device = int(device)
+    return g
+
+
+def make_params(**kw):
+    p = nyxrt_params()
+    for k, v in kw.items():
+        setattr(p, k, v)
+    return p
+
+
+class Tracer:
+    """Owns a context and its torch-allocated workspace."""
+
+    def __init__(self, shape_zyx, dx_cm, params, field_dtype=torch.float64, max_sources=1, batch_rays=0,
+                 host_staging=False, device=0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("nyxrt needs a CUDA device; there is no CPU fallback")
+        self.grid = make_grid(shape_zyx, dx_cm, field_dtype, device=device)
+        self.params = make_params(**params)
+        self.shape = tuple(int(v) for v in shape_zyx)
+        self.device = torch.device("cuda", device)
+        self.ctx = nyxrt_create(self.grid, self.params)
+        self.max_sources = max(int(max_sources), 1)
+        nbytes = nyxrt_workspace_bytes(self.ctx, self.max_sources, batch_rays, host_staging)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        nyxrt_set_workspace(self.ctx, self.workspace, self.max_sources, batch_rays, host_staging)
+
+    def set_fields(self, nH, xHI, stream=None):
+        self._fields = (nH, xHI)            # keep the borrowed tensors alive
+        nyxrt_set_fields(self.ctx, nH, xHI, stream)
+
+    def set_sources(self, pos, L, stream=None):
+        nyxrt_set_sources(self.ctx, pos, L, stream)
+
+    def trace(self, gamma=None, heat=None, want_heat=True, stream=None):
+        if gamma is None:
+            gamma = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        if heat is None and want_heat:
+            heat = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        st = nyxrt_trace(self.ctx, gamma, heat, stream)
+        return gamma, heat, st
+
+    def catalog(self):
+        return nyxrt_get_catalog(self.ctx)
+
+    def step_host(self, nH, xHI, pos, L, gamma, heat=None):
+        return nyxrt_step_host(self.ctx, nH, xHI, pos, L, gamma, heat)
+
+    def pix2dir(self, level, pix_begin, n):
+        return nyxrt_pix2dir(self.ctx, level, pix_begin, n)
+
+    def close(self):
+        if self.ctx is not None:
+            nyxrt_destroy(self.ctx)
+            self.ctx = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
