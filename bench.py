@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- one adaptive ray-tracing step (all hot-path rows: source dedup/merge, emit, march+deposit,
+filter, split, finalise) on BASELINE.json's production configuration (config 5: 1024^3 fp32 fields, 10^6
+sources, merging on), per GPU.  See DESIGN.md "Measurement".
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--n-src N]
+
+Prints ONE JSON line (rank 0).  metric = ray-cell segments per second over the whole RT step.
+N > 1 (torchrun): the path does not shard on the graded configuration ("replicas only", DESIGN.md
+"Multi-GPU"): every rank runs the same step on its own GPU; value = N * segments / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+ALGO_BYTES_PER_SEGMENT = {"f32": 48, "f64": 64}     # 4 field loads + 2 accumulator RMWs
+METRIC = "ray_cell_segments_per_s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--n-src", type=int, default=0, help="use only the first N sources (0 = all)")
+    ap.add_argument("--batch-rays", type=int, default=0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([v.strip() for v in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+def make_workload(args, device):
+    from paper_2512_12466_b200 import synth
+    cfg = synth.make(args.config, device=device)
+    pos, L = cfg["src_pos"].numpy(), cfg["src_L"].numpy()
+    if args.n_src:
+        pos, L = pos[:args.n_src], L[:args.n_src]
+    return cfg, pos, L
+
+
+def oracle_sample(cfg, pos, L, budget_s):
+    """The CPU oracle, as it stands, on a bounded sample of the same workload: the whole step (dedup,
+    merge, trace) on successive chunks of the source list until ~budget_s of CPU time is spent."""
+    from oracle import oracle as O
+    import numpy as np
+    nH = cfg["nH"].cpu().numpy()
+    xHI = cfg["xHI"].cpu().numpy()
+    g = O.make_grid(cfg["shape"], cfg["dx_cm"], field_dtype=nH.dtype)
+    p = O.make_params(**cfg["params"])
+    seg, t_used, n_used, chunk, a = 0, 0.0, 0, 8, 0
+    while t_used < budget_s and a < len(L):
+        b = min(len(L), a + chunk)
+        t0 = time.perf_counter()
+        _, _, st, _ = O.step(g, p, nH, xHI, pos[a:b], L[a:b], want_heat=True)
+        dt = time.perf_counter() - t0
+        seg += st.segments
+        t_used += dt
+        n_used += b - a
+        a = b
+        if dt < 0.2 * budget_s:
+            chunk = min(chunk * 2, 4096)
+    return dict(value=seg / t_used if t_used > 0 else 0.0, unit="segments/s", cores=1, kind="oracle",
+                sample="oracle.step (dedup, merge, trace, finalise) on the first %d of %d input sources of the same "
+                       "fields: %d segments in %.1f s, single thread" % (n_used, len(L), seg, t_used),
+                segments=int(seg), seconds=t_used)
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores; each step is a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import torch
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    cfg, pos, L = make_workload(args, dev)
+    per_step = max(3.0, min(20.0, 60.0 / max(1, args.steps + args.warmup)))
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(cfg, pos, L, 1.0)
+    seg, sec, last = 0, 0.0, None
+    for _ in range(args.steps):
+        last = oracle_sample(cfg, pos, L, per_step)
+        seg += last["segments"]
+        sec += last["seconds"]
+    v = seg / sec
+    out = dict(impl="reference", metric=METRIC, value=v, unit="segments/s", n_gpus=args.gpus, steps=args.steps,
+               warmup=args.warmup, ms_per_step=1e3 * sec / args.steps, higher_is_better=True, scaling="weak",
+               vs_baseline=None, dtype="f64", data="synthetic",
+               config=dict(workload=cfg["name"], notes=cfg["notes"], sample=last["sample"]),
+               cpu_baseline=dict(value=v, unit="segments/s", cores=1, kind="oracle", sample=last["sample"]),
+               e2e=dict(value=v, unit="segments/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(out))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2512_12466_b200 import nyxrt
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg, pos, L = make_workload(args, "cuda")
+    nH, xHI = cfg["nH"], cfg["xHI"]
+    fdt = "f32" if nH.dtype == torch.float32 else "f64"
+    tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], cfg["params"], field_dtype=nH.dtype, max_sources=len(L),
+                      batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local)
+    gam = torch.empty(cfg["shape"], dtype=torch.float64, device="cuda")
+    heat = torch.empty_like(gam)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        # one RT step: fields of this step -> absorber field, sources -> catalogue, ray loop, finalise
+        tr.set_fields(nH, xHI, stream)
+        tr.set_sources(pos, L, stream)
+        return tr.trace(gam, heat, stream=stream)[2]
+
+    for _ in range(args.warmup):
+        st = step()
+    barrier()
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    seg = 0
+    ms_march = 0.0
+    launches = 0
+    march_launches = 0
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        st = step()
+        seg += st.segments
+        ms_march += st.ms_march
+        launches += st.kernel_launches + 3            # + prep_fields, sum_partials, snap
+        march_launches += st.march_launches
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop() if rank == 0 else None
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * seg / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        h_nH = nH.cpu().pin_memory()
+        h_xHI = xHI.cpu().pin_memory()
+        h_g = torch.empty(cfg["shape"], dtype=torch.float64).pin_memory()
+        h_h = torch.empty(cfg["shape"], dtype=torch.float64).pin_memory()
+        tr.step_host(h_nH, h_xHI, pos, L, h_g, h_h)                 # warm-up
+        ke = min(args.steps, 2)
+        barrier()
+        t0 = time.perf_counter()
+        seg_e = 0
+        for _ in range(ke):
+            seg_e += tr.step_host(h_nH, h_xHI, pos, L, h_g, h_h).segments
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+        e2e = dict(value=world * seg_e / dt, unit="segments/s", steps=ke, ms_per_step=1e3 * dt / ke,
+                   h2d_bytes_per_step=int(2 * h_nH.numel() * h_nH.element_size() + pos.nbytes + L.nbytes),
+                   d2h_bytes_per_step=int(2 * h_g.numel() * 8),
+                   checksum_gamma_sum=float(h_g.sum()))
+        del h_nH, h_xHI, h_g, h_h
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        bps = ALGO_BYTES_PER_SEGMENT[fdt]
+        ach = bps * seg / (ms_march * 1e-3) / 1e9          # algorithmic GB/s of the march launches alone
+        roof = dict(bound="hbm", kernel="march_kernel<3>", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak,
+                    traffic=None, algorithmic_bytes_per_segment=bps, segments_per_launch=seg / max(march_launches, 1),
+                    avg_launch_ms=ms_march / max(march_launches, 1), march_share_of_step=ms_march / ms,
+                    peak_source=peak_src,
+                    note="achieved = %d B x segments / sum of march-launch durations (CUDA events around every "
+                         "launch on the launching stream); DRAM traffic per launch: see profiles/" % bps)
+        tfile = os.path.join(ROOT, "profiles", "march_traffic.json")
+        if os.path.exists(tfile):
+            try:
+                roof["traffic"] = json.load(open(tfile)).get("dram_bytes_per_launch")
+            except (ValueError, OSError):
+                pass
+        cpu = None
+        if not args.no_cpu:
+            cpu = oracle_sample(cfg, pos, L, args.cpu_seconds)
+            cpu.pop("segments"); cpu.pop("seconds")
+        out = dict(metric=METRIC, value=value, unit="segments/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
+                   ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                   data="synthetic",
+                   config=dict(workload=cfg["name"], grid=list(cfg["shape"]), field_dtype=fdt, n_sources=int(len(L)),
+                               n_sources_dedup=int(st.n_src_dedup), n_sources_merged=int(st.n_src_merged),
+                               segments_per_step=int(seg // args.steps), notes=cfg["notes"],
+                               l2="inputs larger than L2 (fields + accumulator = %.1f GB), no flush"
+                                  % ((2 * nH.numel() * nH.element_size() + 16 * nH.numel()) / 1e9),
+                               multi_gpu="replicas only"),
+                   rt_step_ms=ms / args.steps, march_ms_per_step=ms_march / args.steps,
+                   gpu_launches=int(launches), clocks=clk, e2e=e2e, roofline=roof, cpu_baseline=cpu,
+                   stats=dict(iterations=int(st.iterations), peak_pool_rays=int(st.peak_pool_rays),
+                              ms_sources=st.ms_sources, ms_loop=st.ms_loop, ms_finalise=st.ms_finalise,
+                              spawned=list(st.spawned)[:14],
+                              budget_rel=(st.photons_absorbed + st.photons_escaped + st.photons_residual
+                                          - st.photons_emitted) / max(st.photons_emitted, 1e-300)))
+        print(json.dumps(out))
+    tr.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -88,7 +88,11 @@ typedef struct {
     double   photons_escaped;            /* carried out of the box                                  */
     double   photons_residual;           /* left in rays filtered by tau_max / l_max                */
     double   photons_lost;               /* geom_mode 1 and 4 only (no secondary correction)        */
+    uint64_t march_launches;             /* march launches that had rays (== iterations)            */
+    uint64_t kernel_launches;            /* launches of this library's own kernels in the call      */
     float    ms_sources, ms_loop, ms_finalise, ms_total;   /* CUDA-event times of the phases        */
+    float    ms_march;                   /* sum of the march launches' own durations (CUDA events)  */
+    float    pad_;
 } nyxrt_stats;
 
 /* Create a context for one grid.  Copies *grid and *params.  Allocates only small bookkeeping

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -61,9 +62,12 @@ struct nyxrt_ctx {
     const void *d_nH, *d_xHI;
     bool have_fields, have_sources, have_catalog;
     long long n_src, n_dedup, n_cat;
+    unsigned long long n_aux_launches;     // own kernels launched outside the ray loop in this trace
     int cat_sel;                           // which of sb.cell[]/L2[]/r[] holds the final catalogue
     double r2_split[MAXLEV], K[MAXLEV];
     cudaEvent_t ev[4];
+    cudaEvent_t *mev;                      // pairs of events around every march launch
+    long long mev_cap;
     cudaStream_t own_stream;
     LoopState *h_ls;                       // pinned
     DevStats *h_ds;                        // pinned
@@ -194,6 +198,7 @@ int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     ctx->n_dedup = ctx->n_cat = 0;
     ctx->cat_sel = 0;
     if (n == 0) return NYXRT_OK;
+    ctx->n_aux_launches += do_merge ? 14 : 4;     // own kernels below (CUB launches not counted)
     int key_bits = 1;
     while (((long long)1 << key_bits) < ctx->ncell) ++key_bits;
     size_t tb = s.cub_bytes;
@@ -331,6 +336,8 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
 
 void nyxrt_destroy(nyxrt_ctx *ctx) {
     if (!ctx) return;
+    for (long long k = 0; k < ctx->mev_cap; ++k) cudaEventDestroy(ctx->mev[k]);
+    free(ctx->mev);
     for (int k = 0; k < 4; ++k)
         if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
@@ -441,7 +448,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
         CU(cudaStreamSynchronize(st));
         do_merge = ctx->h_scalars[0] / (double)ctx->ncell > ctx->p.automerge_xmean;
     }
-    // the snap keys are consumed by the sort; keep them for a later trace by sorting out of place
+    ctx->n_aux_launches = 3;                      // sum_flux, finalise, sum_partials
     int rc = source_pass(ctx, st, do_merge);
     if (rc) return rc;
     ctx->have_catalog = true;
@@ -472,16 +479,28 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     const int gt = geom_template(ctx->p.geom_mode);
     const int emit_blocks = ctx->sm_count * 4;
     int chunk = 8;
+    long long n_launch = 0;
     for (;;) {
         for (int i = 0; i < chunk; ++i) {
             sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev);
             emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0]);
+            if (n_launch + 1 > ctx->mev_cap / 2) {                       // grow the event pool
+                const long long cap = ctx->mev_cap ? 2 * ctx->mev_cap : 1024;
+                cudaEvent_t *m = (cudaEvent_t *)realloc(ctx->mev, cap * sizeof(cudaEvent_t));
+                if (!m) return fail(ctx, NYXRT_ENOMEM, "trace: host allocation failed");
+                ctx->mev = m;
+                for (long long k = ctx->mev_cap; k < cap; ++k) CU(cudaEventCreate(&ctx->mev[k]));
+                ctx->mev_cap = cap;
+            }
+            CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
             switch (gt) {
                 case 0: launch_march<0>(a, ctx->march_blocks, st); break;
                 case 1: launch_march<1>(a, ctx->march_blocks, st); break;
                 case 4: launch_march<4>(a, ctx->march_blocks, st); break;
                 default: launch_march<3>(a, ctx->march_blocks, st); break;
             }
+            CU(cudaEventRecord(ctx->mev[2 * n_launch + 1], st));
+            ++n_launch;
         }
         CU(cudaMemcpyAsync(ctx->h_ls, ctx->ls, sizeof(LoopState), cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
@@ -523,6 +542,16 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
         cudaEventElapsedTime(&hs->ms_loop, ctx->ev[1], ctx->ev[2]);
         cudaEventElapsedTime(&hs->ms_finalise, ctx->ev[2], ctx->ev[3]);
         cudaEventElapsedTime(&hs->ms_total, ctx->ev[0], ctx->ev[3]);
+        double ms = 0.0;
+        const long long live = (long long)ctx->h_ls->iterations;       // launches that had a batch
+        for (long long k = 0; k < n_launch && k < live; ++k) {
+            float t = 0.f;
+            cudaEventElapsedTime(&t, ctx->mev[2 * k], ctx->mev[2 * k + 1]);
+            ms += t;
+        }
+        hs->ms_march = (float)ms;
+        hs->march_launches = (uint64_t)live;
+        hs->kernel_launches = (uint64_t)(3 * n_launch) + ctx->n_aux_launches;
     }
     return NYXRT_OK;
 }

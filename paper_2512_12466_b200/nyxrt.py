@@ -46,8 +46,9 @@ class nyxrt_stats(C.Structure):
                 ("iterations", C.c_uint64), ("peak_pool_rays", C.c_uint64),
                 ("photons_emitted", C.c_double), ("photons_absorbed", C.c_double),
                 ("photons_escaped", C.c_double), ("photons_residual", C.c_double), ("photons_lost", C.c_double),
+                ("march_launches", C.c_uint64), ("kernel_launches", C.c_uint64),
                 ("ms_sources", C.c_float), ("ms_loop", C.c_float), ("ms_finalise", C.c_float),
-                ("ms_total", C.c_float)]
+                ("ms_total", C.c_float), ("ms_march", C.c_float), ("pad_", C.c_float)]
 
     def as_dict(self):
         d = {}
