@@ -1,10 +1,17 @@
-// The ray loop on the device: scheduler, emit, march+deposit+filter+split (SURVEY/DESIGN rows a4-a8).
+// The ray loop on the device: scheduler, emit, march+deposit+filter+split (DESIGN.md rows a4-a8), field
+// preparation and finalise (a9).
 //
 // One launch marches a batch of rays that all sit on the SAME HEALPix level (the pool is one stack per
 // level), so the split radius, the pixel width and the expected number of cells per ray are uniform
 // across a launch.  Each ray is marched to its end: tau >= tau_max (filter), box exit
 // (BASELINE.json configs; reading R20) or the split criterion Eq. 4, in which case the
 // four children are pushed on the stack of level+1.
+//
+// Kernel shape (sm_100a, issue-bound rather than HBM-bound, see profiles/): persistent warps.  A warp claims
+// chunks of rays, initialises 32 at a time with all lanes active (HEALPix direction, start cell), parks
+// them in a shared-memory queue, and its lanes pop a new ray whenever theirs ends, so ray-length tails do
+// not idle lanes.  The grids are padded by one halo cell holding -inf: leaving the box is "the absorber I
+// just loaded is -inf", a neighbour outside the box is never eligible, and no cell coordinates are tracked.
 //
 // Everything that steers control flow follows DESIGN.md's DEC list literally; this translation unit is
 // compiled with -fmad=false.
@@ -15,17 +22,20 @@
 namespace nyxrt {
 
 constexpr int MARCH_THREADS = 256;
+constexpr int MARCH_WARPS = MARCH_THREADS / 32;
+constexpr int QCAP = 64;                 // queue entries per warp (power of two, >= 2 * 32)
 
 // ---------------------------------------------------------------------------------------------------
 // Scheduler: one thread decides what the next emit + march launches do.
 //   1. deepest level holding a full batch; else
 //   2. if sources remain, top level 0 up with 12 rays per source, then 1. again; else
 //   3. the shallowest non-empty level (drain).
-// With caps of 2B (level 0) and 5B (deeper levels) no stack can overflow.
+// With caps of 2B (level 0) and 5B + slab slack (deeper levels) no stack can overflow.
 __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     ls->emit_n = 0;
     ls->batch = 0;
+    ls->fetch = 0;
     if (ls->done) return;
     const long long B = ls->batch_rays;
     int pick = -1;
@@ -62,8 +72,9 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->level = pick;
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
+    ls->seg_round = pick < 2 ? 1 : (pick < 4 ? 2 : 4);
     ls->iterations += 1;
-    ds->spawned[pick] += (unsigned long long)b;          // every ray is marched exactly once
+    ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -83,142 +94,102 @@ __global__ void emit_kernel(const LoopState *ls, RayPool pool, const double *cat
 }
 
 // ---------------------------------------------------------------------------------------------------
-// exp(-x) and 1 - exp(-x) for x >= 0, each to a few ulp (not DEC: tolerance 1e-9).
-__device__ __forceinline__ void absorb_fraction(double dtau, double &gone, double &left) {
-    gone = -expm1(-dtau);                      // Eq. 1's (1 - e^-dtau), accurate for thin cells
-    left = (dtau < 0.5) ? (1.0 - gone) : exp(-dtau);
+// exp(-x) and 1 - exp(-x) for x >= 0 in one pass (not DEC: the tolerance is 1e-9).
+// x = k ln2 + r, |r| <= ln2/2; e^-r - 1 by its Taylor series through r^13 (remainder < 1e-17 relative);
+// left = 2^-k (1 + p), gone = 1 - left = -(2^-k p + (2^-k - 1)) with both terms exact up to one rounding,
+// so thin cells (k = 0, gone = -p = x - x^2/2 + ...) keep full relative accuracy where 1 - exp(-x) would not.
+__device__ __forceinline__ void absorb_fraction(double x, double &gone, double &left) {
+    if (x > 690.0) { gone = 1.0; left = 0.0; return; }
+    const double MAGIC = 6755399441055744.0;                     // 1.5 * 2^52: round to nearest integer
+    const double kd_m = fma(x, 1.4426950408889634, MAGIC);
+    const int k = __double2loint(kd_m);                          // 0 .. 996
+    const double kd = kd_m - MAGIC;
+    double r = fma(kd, -6.93147180369123816490e-01, x);          // ln2 hi
+    r = fma(kd, -1.90821492927058770002e-10, r);                 // ln2 lo
+    const double t = -r;
+    double q = 1.0 / 6227020800.0;                               // 1/13!
+    q = fma(q, t, 1.0 / 479001600.0);
+    q = fma(q, t, 1.0 / 39916800.0);
+    q = fma(q, t, 1.0 / 3628800.0);
+    q = fma(q, t, 1.0 / 362880.0);
+    q = fma(q, t, 1.0 / 40320.0);
+    q = fma(q, t, 1.0 / 5040.0);
+    q = fma(q, t, 1.0 / 720.0);
+    q = fma(q, t, 1.0 / 120.0);
+    q = fma(q, t, 1.0 / 24.0);
+    q = fma(q, t, 1.0 / 6.0);
+    q = fma(q, t, 0.5);
+    const double p = fma(t * t, q, t);                           // e^t - 1
+    const double sc = __hiloint2double((1023 - k) << 20, 0);     // 2^-k
+    left = fma(sc, p, sc);
+    gone = -fma(sc, p, sc - 1.0);
+}
+
+// a / b to ~1 ulp without the IEEE slow path (not DEC: only scales a deposit); b is a positive normal number
+__device__ __forceinline__ double div_fast(double a, double b) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
+    double e = fma(-b, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-b, y, 1.0);
+    y = fma(y, e, y);
+    const double qv = a * y;
+    return fma(fma(-b, qv, a), y, qv);
 }
 
 enum { OUT_NONE = 0, OUT_SPLIT = 1, OUT_KILL_TAU = 2, OUT_EXIT = 3, OUT_KILL_LMAX = 4 };
 
+// shared-memory queue of initialised rays, one per warp, structure of arrays
+struct WarpQueue {
+    unsigned long long key[QCAP];
+    double s[QCAP], tau[QCAP], N[QCAP];
+    double d[3][QCAP], inv[3][QCAP], od[3][QCAP];
+    long long c[QCAP];
+    int up[QCAP];
+};
+
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
-template <int GEOM>
-__global__ void __launch_bounds__(MARCH_THREADS) march_kernel(const __grid_constant__ MarchArgs A) {
+template <int GEOM, typename IDX>
+__global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_constant__ MarchArgs A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     const LoopState *ls = A.ls;
     const long long batch = ls->batch;
     if (batch == 0) return;
     const int level = ls->level;
+    const int seg_round = ls->seg_round;
     const long long begin = ls->begin;
     const int lane = threadIdx.x & 31;
-    const double r2s = A.r2_split[level], Kl = A.K[level];
-    const long long sy = A.nx, sz = (long long)A.nx * A.ny;
+    const unsigned lt = (1u << lane) - 1u;
+    WarpQueue &Q = reinterpret_cast<WarpQueue *>(smem_raw)[threadIdx.x >> 5];
+    const double r2s = A.r2_split[level], Kl = A.K[level], Kh = 0.5 * A.K[level];
+    const double tau_max = A.tau_max, sdx = A.sdx;
+    const IDX sy = (IDX)A.px, sz = (IDX)A.pxy;
+    const double *__restrict__ absorber = A.absorber;
+    double *__restrict__ acc = A.acc;
 
-    unsigned long long n_seg = 0, n_zero = 0;
-    unsigned int n_split = 0, n_ktau = 0, n_exit = 0, n_klmax = 0;      // lane 0 accumulates warp totals
+    unsigned int n_seg = 0, n_zero = 0;
+    unsigned int n_split = 0, n_ktau = 0, n_exit = 0, n_klmax = 0, n_hole = 0;   // lane 0 holds warp totals
     double esc = 0.0, res = 0.0, lost = 0.0;
 
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    const long long nround = (batch + stride - 1) / stride;
-    for (long long it = 0; it < nround; ++it) {
-        const long long r = it * stride + (long long)blockIdx.x * blockDim.x + threadIdx.x;
-        const bool valid = r < batch;
-        int outcome = OUT_NONE;
-        uint64_t key = 0;
-        double s = 0.0, tau = 0.0, N = 0.0;
-        if (valid) {
-            key = A.pool.key[begin + r];
-            s = A.pool.s[begin + r];
-            tau = A.pool.tau[begin + r];
-            N = A.pool.N[begin + r];
-            const int4 sc = A.cat_cell[key_src(key)];
-            double d0, d1, d2;
-            pix2dir(level, key_pix(key), d0, d1, d2);
-            // O4: start-of-life cell, source-relative (source at its cell centre)
-            double q, fl, inv0, inv1, inv2, sx0, sx1, sx2;
-            int o0, o1, o2;
-            q = fma(s, d0, 0.5); fl = floor(q); o0 = (int)fl; if (q == fl && d0 < 0.0) o0 -= 1;
-            q = fma(s, d1, 0.5); fl = floor(q); o1 = (int)fl; if (q == fl && d1 < 0.0) o1 -= 1;
-            q = fma(s, d2, 0.5); fl = floor(q); o2 = (int)fl; if (q == fl && d2 < 0.0) o2 -= 1;
-            const int st0 = d0 > 0.0 ? 1 : -1, st1 = d1 > 0.0 ? 1 : -1, st2 = d2 > 0.0 ? 1 : -1;
-            const int up0 = d0 > 0.0 ? 1 : 0, up1 = d1 > 0.0 ? 1 : 0, up2 = d2 > 0.0 ? 1 : 0;
-            if (d0 == 0.0) { inv0 = 0.0; sx0 = CUDART_INF; } else { inv0 = 1.0 / d0; sx0 = ((double)(o0 + up0) - 0.5) * inv0; }
-            if (d1 == 0.0) { inv1 = 0.0; sx1 = CUDART_INF; } else { inv1 = 1.0 / d1; sx1 = ((double)(o1 + up1) - 0.5) * inv1; }
-            if (d2 == 0.0) { inv2 = 0.0; sx2 = CUDART_INF; } else { inv2 = 1.0 / d2; sx2 = ((double)(o2 + up2) - 0.5) * inv2; }
-            int ci = sc.x + o0, cj = sc.y + o1, ck = sc.z + o2;
-            if ((unsigned)ci >= (unsigned)A.nx || (unsigned)cj >= (unsigned)A.ny || (unsigned)ck >= (unsigned)A.nz) {
-                outcome = OUT_EXIT;
-            } else if (tau >= A.tau_max) {
-                outcome = OUT_KILL_TAU;
-            } else if (level >= A.level_max) {
-                outcome = OUT_KILL_LMAX;
-            } else {
-                long long c = ((long long)ck * A.ny + cj) * A.nx + ci;
-                for (;;) {
-                    if (tau >= A.tau_max) { outcome = OUT_KILL_TAU; break; }       // 1. filter
-                    if (s * s > r2s) { outcome = OUT_SPLIT; break; }               // 3. Eq. 4
-                    // 4. one cell
-                    int ax = 0;
-                    double s_exit = sx0;
-                    if (sx1 < s_exit) { s_exit = sx1; ax = 1; }
-                    if (sx2 < s_exit) { s_exit = sx2; ax = 2; }
-                    double ds = s_exit - s;
-                    if (!(ds > 0.0)) ds = 0.0;
-                    if (ds > 0.0) {
-                        ++n_seg;
-                        const double a_c = fabs(__ldg(A.absorber + c));
-                        const double dtau = (a_c * A.sdx) * ds;
-                        double gone, left;
-                        absorb_fraction(dtau, gone, left);
-                        const double dN = N * gone;
-                        if (dN > 0.0) {
-                            double fc = 1.0;
-                            long long cn = -1;
-                            if (GEOM != 0) {
-                                const double s_m = s + 0.5 * ds;
-                                double m0 = fma(s_m, d0, 0.5) - (double)o0;
-                                double m1 = fma(s_m, d1, 0.5) - (double)o1;
-                                double m2 = fma(s_m, d2, 0.5) - (double)o2;
-                                m0 = m0 < 0.0 ? 0.0 : (m0 > 1.0 ? 1.0 : m0);
-                                m1 = m1 < 0.0 ? 0.0 : (m1 > 1.0 ? 1.0 : m1);
-                                m2 = m2 < 0.0 ? 0.0 : (m2 > 1.0 ? 1.0 : m2);
-                                double de = m0; int face = 0;                      // first minimum, order x-,x+,y-,y+,z-,z+
-                                double t = 1.0 - m0; if (t < de) { de = t; face = 1; }
-                                if (m1 < de) { de = m1; face = 2; }
-                                t = 1.0 - m1; if (t < de) { de = t; face = 3; }
-                                if (m2 < de) { de = m2; face = 4; }
-                                t = 1.0 - m2; if (t < de) { de = t; face = 5; }
-                                const double l_pix = s_m * Kl;
-                                if (de < 0.5 * l_pix) {                            // Eq. 5 / 7, first condition
-                                    if (GEOM == 1) fc = 0.5 + de / l_pix;
-                                    else if (GEOM == 4) { fc = 0.5 + de / l_pix; fc = fc * fc; }
-                                    else {
-                                        const int fa = face >> 1, dir = (face & 1) ? 1 : -1;
-                                        const int ni = ci + (fa == 0 ? dir : 0), nj = cj + (fa == 1 ? dir : 0),
-                                                  nk = ck + (fa == 2 ? dir : 0);
-                                        if ((unsigned)ni < (unsigned)A.nx && (unsigned)nj < (unsigned)A.ny &&
-                                            (unsigned)nk < (unsigned)A.nz) {
-                                            const long long cq = c + (fa == 0 ? dir : (fa == 1 ? dir * sy : dir * sz));
-                                            const double a_n = __ldg(A.absorber + cq);   // > 0: absorber present and n_H >= n_th
-                                            if (a_n > 0.0) { fc = 0.5 + de / l_pix; cn = cq; }
-                                        }
-                                    }
-                                }
-                            }
-                            atomicAdd(A.acc + c, fc * dN);
-                            if (GEOM == 3) {
-                                if (cn >= 0) atomicAdd(A.acc + cn, (1.0 - fc) * dN);
-                            } else if (GEOM == 1 || GEOM == 4) {
-                                lost += (1.0 - fc) * dN;
-                            }
-                        }
-                        N = N * left;
-                        tau = tau + dtau;
-                    } else {
-                        ++n_zero;
-                    }
-                    s = s_exit;
-                    if (ax == 0) { o0 += st0; ci += st0; c += st0; sx0 = ((double)(o0 + up0) - 0.5) * inv0;
-                                   if ((unsigned)ci >= (unsigned)A.nx) { outcome = OUT_EXIT; break; } }
-                    else if (ax == 1) { o1 += st1; cj += st1; c += st1 * sy; sx1 = ((double)(o1 + up1) - 0.5) * inv1;
-                                   if ((unsigned)cj >= (unsigned)A.ny) { outcome = OUT_EXIT; break; } }
-                    else { o2 += st2; ck += st2; c += st2 * sz; sx2 = ((double)(o2 + up2) - 0.5) * inv2;
-                                   if ((unsigned)ck >= (unsigned)A.nz) { outcome = OUT_EXIT; break; } }
-                }
-            }
-            if (outcome == OUT_EXIT) esc += N;
-            else if (outcome == OUT_KILL_TAU || outcome == OUT_KILL_LMAX) res += N;
-        }
-        // warp-converged epilogue: counters and child allocation
+    // warp-uniform bookkeeping
+    int qhead = 0, qcount = 0;
+    long long chunk_pos = 0, chunk_end = 0;
+    bool exhausted = false;
+    long long slab_pos = 0, slab_end = 0;          // child slots reserved on the stack of level+1
+
+    // per-lane ray state
+    bool has = false;
+    unsigned long long key = 0;
+    double s = 0.0, tau = 0.0, N = 0.0;
+    double d0 = 0, d1 = 0, d2 = 0, inv0 = 0, inv1 = 0, inv2 = 0, od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
+    double a_raw = 0.0;
+    IDX c = 0, cs0 = 0, cs1 = 0, cs2 = 0;
+    int up = 0;
+
+    // retire rays whose outcome is known (all lanes call it; outcome NONE = nothing to do)
+    auto retire = [&](int outcome, unsigned long long rkey, double rs, double rtau, double rN) {
+        const unsigned m_any = __ballot_sync(0xffffffffu, outcome != OUT_NONE);
+        if (m_any == 0) return;
         const unsigned m_split = __ballot_sync(0xffffffffu, outcome == OUT_SPLIT);
         const unsigned m_ktau = __ballot_sync(0xffffffffu, outcome == OUT_KILL_TAU);
         const unsigned m_exit = __ballot_sync(0xffffffffu, outcome == OUT_EXIT);
@@ -226,44 +197,225 @@ __global__ void __launch_bounds__(MARCH_THREADS) march_kernel(const __grid_const
         if (lane == 0) {
             n_split += __popc(m_split); n_ktau += __popc(m_ktau); n_exit += __popc(m_exit); n_klmax += __popc(m_klmax);
         }
+        if (outcome == OUT_EXIT) esc += rN;
+        else if (outcome == OUT_KILL_TAU || outcome == OUT_KILL_LMAX) res += rN;
         if (m_split) {
-            long long base = 0;
-            const int nsp = __popc(m_split);
-            if (lane == 0) base = atomicAdd((unsigned long long *)&A.ls->count[level + 1], (unsigned long long)(4 * nsp));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (base + 4 * nsp > A.pool.cap[level + 1]) {
-                if (lane == 0) A.ls->overflow = 1;
-            } else if (outcome == OUT_SPLIT) {
-                const long long w = A.pool.off[level + 1] + base + 4 * __popc(m_split & ((1u << lane) - 1u));
-                const uint32_t src = key_src(key), p4 = 4u * key_pix(key);
-                const double Nc = N * 0.25;                                      // L shared evenly
+            const int need = 4 * __popc(m_split);
+            if (slab_pos + need > slab_end) {
+                // pad the rest of the old slab with holes, reserve a new one
+                for (long long h = slab_pos + lane; h < slab_end; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
+                long long base = 0;
+                if (lane == 0) base = (long long)atomicAdd((unsigned long long *)&A.ls->count[level + 1],
+                                                           (unsigned long long)CHILD_SLAB);
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (base + CHILD_SLAB > A.pool.cap[level + 1]) {
+                    if (lane == 0) A.ls->overflow = 1;
+                    slab_pos = slab_end = 0;
+                    return;
+                }
+                slab_pos = base;
+                slab_end = base + CHILD_SLAB;
+            }
+            if (outcome == OUT_SPLIT) {
+                const long long w = A.pool.off[level + 1] + slab_pos + 4 * __popc(m_split & lt);
+                const uint32_t src = key_src(rkey), p4 = 4u * key_pix(rkey);
+                const double Nc = rN * 0.25;                                     // L shared evenly
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     A.pool.key[w + k] = ray_key(src, level + 1, p4 + k);
-                    A.pool.s[w + k] = s;
-                    A.pool.tau[w + k] = tau;
+                    A.pool.s[w + k] = rs;
+                    A.pool.tau[w + k] = rtau;
                     A.pool.N[w + k] = Nc;
                 }
             }
+            slab_pos += need;
         }
+    };
+
+    for (;;) {
+        // ---- top up the queue: 32 rays at a time, all lanes active --------------------------------
+        while (qcount <= QCAP - 32 && !exhausted) {
+            if (chunk_pos >= chunk_end) {
+                unsigned long long f = 0;
+                if (lane == 0) f = atomicAdd((unsigned long long *)&A.ls->fetch, (unsigned long long)FETCH_CHUNK);
+                f = __shfl_sync(0xffffffffu, f, 0);
+                if ((long long)f >= batch) { exhausted = true; break; }
+                chunk_pos = (long long)f;
+                chunk_end = chunk_pos + FETCH_CHUNK < batch ? chunk_pos + FETCH_CHUNK : batch;
+            }
+            const long long r = chunk_pos + lane;
+            chunk_pos += 32;
+            int outcome = OUT_NONE;
+            bool march = false;
+            unsigned long long ikey = KEY_HOLE;
+            double is = 0.0, itau = 0.0, iN = 0.0;
+            if (r < chunk_end) ikey = A.pool.key[begin + r];
+            const bool real = ikey != KEY_HOLE;
+            const unsigned m_hole = __ballot_sync(0xffffffffu, r < chunk_end && !real);
+            if (lane == 0) n_hole += __popc(m_hole);
+            double e0 = 0, e1 = 0, e2 = 0, i0 = 0, i1 = 0, i2 = 0, f0 = 0, f1 = 0, f2 = 0;
+            long long ic = 0;
+            int iup = 0;
+            if (real) {
+                is = A.pool.s[begin + r];
+                itau = A.pool.tau[begin + r];
+                iN = A.pool.N[begin + r];
+                const int4 sc = A.cat_cell[key_src(ikey)];
+                pix2dir(level, key_pix(ikey), e0, e1, e2);
+                // O4: start-of-life cell, source-relative (source at its cell centre)
+                double q;
+                q = fma(is, e0, 0.5); f0 = floor(q); if (q == f0 && e0 < 0.0) f0 -= 1.0;
+                q = fma(is, e1, 0.5); f1 = floor(q); if (q == f1 && e1 < 0.0) f1 -= 1.0;
+                q = fma(is, e2, 0.5); f2 = floor(q); if (q == f2 && e2 < 0.0) f2 -= 1.0;
+                iup = (e0 > 0.0 ? 1 : 0) | (e1 > 0.0 ? 2 : 0) | (e2 > 0.0 ? 4 : 0);
+                i0 = (e0 == 0.0) ? -CUDART_INF : 1.0 / e0;                   // with od + (-0.5): s_x = +inf
+                i1 = (e1 == 0.0) ? -CUDART_INF : 1.0 / e1;
+                i2 = (e2 == 0.0) ? -CUDART_INF : 1.0 / e2;
+                const long long ci = sc.x + (long long)f0, cj = sc.y + (long long)f1, ck = sc.z + (long long)f2;
+                if (ci < 0 || ci >= A.nx || cj < 0 || cj >= A.ny || ck < 0 || ck >= A.nz) outcome = OUT_EXIT;
+                else if (itau >= tau_max) outcome = OUT_KILL_TAU;
+                else if (level >= A.level_max) outcome = OUT_KILL_LMAX;
+                else if (is * is > r2s) outcome = OUT_SPLIT;
+                else { march = true; ic = ((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1); }
+            }
+            retire(outcome, ikey, is, itau, iN);
+            const unsigned mm = __ballot_sync(0xffffffffu, march);
+            if (march) {
+                const int slot = (qhead + qcount + __popc(mm & lt)) & (QCAP - 1);
+                Q.key[slot] = ikey; Q.s[slot] = is; Q.tau[slot] = itau; Q.N[slot] = iN;
+                Q.d[0][slot] = e0; Q.d[1][slot] = e1; Q.d[2][slot] = e2;
+                Q.inv[0][slot] = i0; Q.inv[1][slot] = i1; Q.inv[2][slot] = i2;
+                Q.od[0][slot] = f0; Q.od[1][slot] = f1; Q.od[2][slot] = f2;
+                Q.c[slot] = ic; Q.up[slot] = iup;
+            }
+            qcount += __popc(mm);
+            __syncwarp();
+        }
+        // ---- idle lanes pop a ray ---------------------------------------------------------------------
+        {
+            const unsigned m_need = __ballot_sync(0xffffffffu, !has);
+            if (m_need != 0 && qcount > 0) {
+                const int rank = __popc(m_need & lt);
+                if (!has && rank < qcount) {
+                    const int slot = (qhead + rank) & (QCAP - 1);
+                    key = Q.key[slot]; s = Q.s[slot]; tau = Q.tau[slot]; N = Q.N[slot];
+                    d0 = Q.d[0][slot]; d1 = Q.d[1][slot]; d2 = Q.d[2][slot];
+                    inv0 = Q.inv[0][slot]; inv1 = Q.inv[1][slot]; inv2 = Q.inv[2][slot];
+                    od0 = Q.od[0][slot]; od1 = Q.od[1][slot]; od2 = Q.od[2][slot];
+                    c = (IDX)Q.c[slot]; up = Q.up[slot];
+                    a_raw = __ldg(absorber + c);
+                    cs0 = (up & 1) ? (IDX)1 : (IDX)-1;
+                    cs1 = (up & 2) ? sy : -sy;
+                    cs2 = (up & 4) ? sz : -sz;
+                    sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0;              // ((o + up) - 0.5) / d
+                    sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1;
+                    sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2;
+                    has = true;
+                }
+                const int want = __popc(m_need);
+                const int taken = want < qcount ? want : qcount;
+                qhead = (qhead + taken) & (QCAP - 1);
+                qcount -= taken;
+            }
+            __syncwarp();
+        }
+        if (__ballot_sync(0xffffffffu, has) == 0) {
+            if (exhausted && qcount == 0) break;
+            continue;
+        }
+        // ---- march: seg_round cells per lane, then retire / refill -------------------------------------
+        int outcome = OUT_NONE;
+        for (int it = 0; it < seg_round; ++it) {
+            if (has && outcome == OUT_NONE) {
+                // geometry of the cell the ray is in (side-effect free, overlaps the absorber load)
+                double s_exit = sx0; int ax = 0;
+                if (sx1 < s_exit) { s_exit = sx1; ax = 1; }
+                if (sx2 < s_exit) { s_exit = sx2; ax = 2; }                       // first minimum, order x, y, z
+                double ds = s_exit - s;
+                if (!(ds > 0.0)) ds = 0.0;
+                bool elig = false;
+                double de = 0.0, s_m = 0.0, a_n = 0.0;
+                IDX cq = c;
+                if (GEOM != 0) {
+                    s_m = s + 0.5 * ds;
+                    double m0 = fma(s_m, d0, 0.5) - od0;
+                    double m1 = fma(s_m, d1, 0.5) - od1;
+                    double m2 = fma(s_m, d2, 0.5) - od2;
+                    m0 = m0 < 0.0 ? 0.0 : (m0 > 1.0 ? 1.0 : m0);
+                    m1 = m1 < 0.0 ? 0.0 : (m1 > 1.0 ? 1.0 : m1);
+                    m2 = m2 < 0.0 ? 0.0 : (m2 > 1.0 ? 1.0 : m2);
+                    de = m0; IDX off = (IDX)-1;                                   // first minimum: x-,x+,y-,y+,z-,z+
+                    double t = 1.0 - m0; if (t < de) { de = t; off = (IDX)1; }
+                    if (m1 < de) { de = m1; off = -sy; }
+                    t = 1.0 - m1; if (t < de) { de = t; off = sy; }
+                    if (m2 < de) { de = m2; off = -sz; }
+                    t = 1.0 - m2; if (t < de) { de = t; off = sz; }
+                    elig = de < s_m * Kh;                                         // D_edge < L_pix / 2  (Eq. 5 / 7)
+                    if (GEOM == 3 && elig && ds > 0.0) { cq = c + off; a_n = __ldg(absorber + cq); }
+                }
+                // order of the tests as in the oracle: box exit, filter, split, then the segment
+                if (a_raw == -CUDART_INF) { outcome = OUT_EXIT; }
+                else if (tau >= tau_max) { outcome = OUT_KILL_TAU; }
+                else if (s * s > r2s) { outcome = OUT_SPLIT; }
+                else {
+                    if (ds > 0.0) {
+                        ++n_seg;
+                        const double a_c = fabs(a_raw);
+                        const double dtau = (a_c * sdx) * ds;
+                        double gone, left;
+                        absorb_fraction(dtau, gone, left);
+                        const double dN = N * gone;
+                        if (dN > 0.0) {
+                            double fc = 1.0;
+                            if (GEOM == 3) {
+                                if (elig && a_n > 0.0) {                          // in the box, absorber > 0, n_H >= n_th
+                                    fc = 0.5 + div_fast(de, s_m * Kl);
+                                    atomicAdd(acc + cq, (1.0 - fc) * dN);
+                                }
+                            } else if (GEOM == 1 || GEOM == 4) {
+                                if (elig) { fc = 0.5 + div_fast(de, s_m * Kl); if (GEOM == 4) fc = fc * fc; }
+                                lost += (1.0 - fc) * dN;
+                            }
+                            atomicAdd(acc + c, fc * dN);
+                        }
+                        N = N * left;
+                        tau = tau + dtau;
+                    } else {
+                        ++n_zero;
+                    }
+                    s = s_exit;
+                    if (ax == 0) { od0 += (up & 1) ? 1.0 : -1.0; c += cs0; sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0; }
+                    else if (ax == 1) { od1 += (up & 2) ? 1.0 : -1.0; c += cs1; sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1; }
+                    else { od2 += (up & 4) ? 1.0 : -1.0; c += cs2; sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2; }
+                    a_raw = __ldg(absorber + c);
+                }
+            }
+        }
+        retire(outcome, key, s, tau, N);
+        if (outcome != OUT_NONE) has = false;
     }
+    // pad the unused tail of the last child slab
+    for (long long h = slab_pos + lane; h < slab_end; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
+
     // flush per-thread / per-warp tallies
+    unsigned long long seg64 = n_seg, zero64 = n_zero;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        n_seg += __shfl_xor_sync(0xffffffffu, n_seg, o);
-        n_zero += __shfl_xor_sync(0xffffffffu, n_zero, o);
+        seg64 += __shfl_xor_sync(0xffffffffu, seg64, o);
+        zero64 += __shfl_xor_sync(0xffffffffu, zero64, o);
         esc += __shfl_xor_sync(0xffffffffu, esc, o);
         res += __shfl_xor_sync(0xffffffffu, res, o);
         lost += __shfl_xor_sync(0xffffffffu, lost, o);
     }
     if (lane == 0) {
         DevStats *ds = A.ds;
-        if (n_seg) atomicAdd(&ds->segments, n_seg);
-        if (n_zero) atomicAdd(&ds->zero_len, n_zero);
+        if (seg64) atomicAdd(&ds->segments, seg64);
+        if (zero64) atomicAdd(&ds->zero_len, zero64);
         if (n_split) atomicAdd(&ds->split[level], (unsigned long long)n_split);
         if (n_ktau) atomicAdd(&ds->killed_tau[level], (unsigned long long)n_ktau);
         if (n_exit) atomicAdd(&ds->exited[level], (unsigned long long)n_exit);
         if (n_klmax) atomicAdd(&ds->killed_lmax[level], (unsigned long long)n_klmax);
+        if (n_hole) atomicAdd(&ds->holes[level], (unsigned long long)n_hole);
         if (esc != 0.0) atomicAdd(&ds->escaped, esc);
         if (res != 0.0) atomicAdd(&ds->residual, res);
         if (lost != 0.0) atomicAdd(&ds->lost, lost);
@@ -271,21 +423,29 @@ __global__ void __launch_bounds__(MARCH_THREADS) march_kernel(const __grid_const
 }
 
 // ---------------------------------------------------------------------------------------------------
-// Field preparation (set_fields): absorber a = n_H x_HI in fp64 (reading R1), with the
-// sign bit carrying Eq. 7-8's "n_H < n_th" so that the march reads ONE value per
-// cell.  Also the per-block partial sums of the ionised fraction 1 - x_HI for automerge.
+// Field preparation (set_fields): absorber a = n_H x_HI in fp64 (reading R1) on the PADDED
+// grid, with the sign bit carrying Eq. 7-8's "n_H < n_th" so that the march reads ONE
+// value per cell, and -inf in the halo.  Also the per-block partial sums of the ionised fraction 1 - x_HI
+// for automerge.
 template <typename T>
 __global__ void prep_fields_kernel(const T *__restrict__ nH, const T *__restrict__ xHI, double *__restrict__ a,
-                                   long long ncell, double n_th, int use_flag, double *__restrict__ partial) {
+                                   int nx, int ny, int nz, double n_th, int use_flag,
+                                   double *__restrict__ partial) {
     __shared__ double sh[256];
     double acc = 0.0;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncell;
-         i += (long long)gridDim.x * blockDim.x) {
-        const double n = (double)nH[i], x = (double)xHI[i];
-        double v = n * x;
-        if (use_flag && !(n >= n_th)) v = -v;
-        a[i] = v;
-        acc += 1.0 - x;
+    const long long px = nx + 2, py = ny + 2, pz = nz + 2, ptot = px * py * pz;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < ptot;
+         q += (long long)gridDim.x * blockDim.x) {
+        const long long i = q % px - 1, j = (q / px) % py - 1, k = q / (px * py) - 1;
+        double v = -CUDART_INF;
+        if (i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz) {
+            const long long t = (k * ny + j) * nx + i;
+            const double n = (double)nH[t], x = (double)xHI[t];
+            v = n * x;
+            if (use_flag && !(n >= n_th)) v = -v;
+            acc += 1.0 - x;
+        }
+        a[q] = v;
     }
     sh[threadIdx.x] = acc;
     __syncthreads();
@@ -312,24 +472,29 @@ __global__ void sum_partials_kernel(const double *partial, int n, double *out) {
 
 // ---------------------------------------------------------------------------------------------------
 // Finalise (row a9): Gamma = photons / (n_HI V) (Eq. 1 with V_box); heating (H1);
-// per-block partial sums of the deposited photons for the budget.
-__global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__ heat,
-                                const double *__restrict__ absorber, long long ncell, double V, double e_excess,
-                                double *__restrict__ partial) {
+// per-block partial sums of the deposited photons for the budget.  Reads the padded accumulator and
+// absorber, writes the caller's dense [nz][ny][nx] outputs.
+__global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__ heat, const double *__restrict__ acc,
+                                const double *__restrict__ absorber, int nx, int ny, int nz, double V,
+                                double e_excess, double *__restrict__ partial) {
     __shared__ double sh[256];
-    double acc = 0.0;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncell;
-         i += (long long)gridDim.x * blockDim.x) {
-        const double ph = gamma[i];
-        acc += ph;
+    double sum = 0.0;
+    const long long ncell = (long long)nx * ny * nz, px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2);
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < ncell;
+         t += (long long)gridDim.x * blockDim.x) {
+        const long long i = t % nx, j = (t / nx) % ny, k = t / ((long long)nx * ny);
+        const long long q = (k + 1) * pxy + (j + 1) * px + (i + 1);
+        const double ph = acc[q];
+        sum += ph;
+        double g = 0.0, h = 0.0;
         if (ph != 0.0) {
-            gamma[i] = ph / (fabs(absorber[i]) * V);
-            if (heat) heat[i] = e_excess * ph / V;
-        } else if (heat) {
-            heat[i] = 0.0;
+            g = ph / (fabs(absorber[q]) * V);
+            h = e_excess * ph / V;
         }
+        gamma[t] = g;
+        if (heat) heat[t] = h;
     }
-    sh[threadIdx.x] = acc;
+    sh[threadIdx.x] = sum;
     __syncthreads();
     for (int o = blockDim.x >> 1; o > 0; o >>= 1) {
         if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];

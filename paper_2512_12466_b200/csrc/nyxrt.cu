@@ -51,7 +51,10 @@ struct nyxrt_ctx {
     uint64_t ws_bytes;
     long long max_sources, batch_rays;
     int host_staging;
-    double *absorber, *partial, *scalars;  // scalars[0] = sum(1-x_HI), [1] = absorbed, [2] = emitted
+    double *absorber, *acc;                // padded grids (nx+2)(ny+2)(nz+2): absorber field, photon accumulator
+    double *partial, *scalars;             // scalars[0] = sum(1-x_HI), [1] = absorbed, [2] = emitted
+    long long pcell;                       // padded cell count
+    bool idx64;                            // padded grid needs 64-bit cell indices
     RayPool pool;
     LoopState *ls;
     DevStats *ds;
@@ -132,7 +135,8 @@ int effective_levels(const nyxrt_ctx *c) {
 uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, int staging) {
     Bump b{static_cast<char *>(base), 0};
     const long long n = max_sources > 0 ? max_sources : 1;
-    c->absorber = b.take<double>(c->ncell);
+    c->absorber = b.take<double>(c->pcell);
+    c->acc = b.take<double>(c->pcell);
     c->partial = b.take<double>(NPARTIAL);
     c->scalars = b.take<double>(8);
     c->ls = b.take<LoopState>(1);
@@ -140,7 +144,8 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
     long long total = 0;
     for (int l = 0; l < MAXLEV; ++l) {
         c->pool.off[l] = total;
-        c->pool.cap[l] = l < c->nlev ? (l == 0 ? 2 * B : 5 * B) : 0;
+        // 2B / 5B bound the rays; the slack holds every warp's partly used child slab
+        c->pool.cap[l] = l < c->nlev ? (l == 0 ? 2 * B : 5 * B + (long long)CHILD_SLAB * c->march_blocks * MARCH_WARPS) : 0;
         total += c->pool.cap[l];
     }
     c->pool.key = b.take<uint64_t>(total);
@@ -183,9 +188,27 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
     return ((b.off + 255) & ~uint64_t(255));
 }
 
+constexpr size_t MARCH_SMEM = sizeof(WarpQueue) * MARCH_WARPS;
+
 template <int GEOM>
-void launch_march(const MarchArgs &a, int blocks, cudaStream_t st) {
-    march_kernel<GEOM><<<blocks, MARCH_THREADS, 0, st>>>(a);
+void launch_march(const MarchArgs &a, bool idx64, int blocks, cudaStream_t st) {
+    if (idx64) march_kernel<GEOM, long long><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+    else march_kernel<GEOM, int><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+}
+
+template <int GEOM>
+cudaError_t setup_march(bool idx64, int *occ) {
+    cudaError_t e;
+    if (idx64) {
+        e = cudaFuncSetAttribute(march_kernel<GEOM, long long>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MARCH_SMEM);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, long long>, MARCH_THREADS, MARCH_SMEM);
+    } else {
+        e = cudaFuncSetAttribute(march_kernel<GEOM, int>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MARCH_SMEM);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, int>, MARCH_THREADS, MARCH_SMEM);
+    }
+    return e;
 }
 
 int geom_template(int mode) { return mode == 2 ? 3 : mode; }
@@ -300,6 +323,8 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     ctx->g = g;
     ctx->p = p;
     ctx->ncell = (long long)g.nx * g.ny * g.nz;
+    ctx->pcell = (long long)(g.nx + 2) * (g.ny + 2) * (g.nz + 2);
+    ctx->idx64 = ctx->pcell >= (1ll << 31);
     const double PI = 0x1.921fb54442d18p+1;
     for (int l = 0; l < MAXLEV; ++l) {
         ctx->r2_split[l] = std::ldexp(3.0 / (PI * p.n_min_ray), 2 * l);   // Eq. 4
@@ -317,10 +342,10 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     int occ = 0;
     if (e == cudaSuccess) {
         switch (geom_template(p.geom_mode)) {
-            case 0: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<0>, MARCH_THREADS, 0); break;
-            case 1: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<1>, MARCH_THREADS, 0); break;
-            case 4: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<4>, MARCH_THREADS, 0); break;
-            default: e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, march_kernel<3>, MARCH_THREADS, 0); break;
+            case 0: e = setup_march<0>(ctx->idx64, &occ); break;
+            case 1: e = setup_march<1>(ctx->idx64, &occ); break;
+            case 4: e = setup_march<4>(ctx->idx64, &occ); break;
+            default: e = setup_march<3>(ctx->idx64, &occ); break;
         }
     }
     if (e != cudaSuccess) {
@@ -389,10 +414,12 @@ int nyxrt_set_fields(nyxrt_ctx *ctx, const void *d_nH, const void *d_xHI, void *
     const int use_flag = ctx->p.geom_mode == 3;
     if (ctx->g.field_dtype)
         prep_fields_kernel<float><<<NPARTIAL, 256, 0, st>>>((const float *)d_nH, (const float *)d_xHI, ctx->absorber,
-                                                            ctx->ncell, ctx->p.n_th, use_flag, ctx->partial);
+                                                            ctx->g.nx, ctx->g.ny, ctx->g.nz, ctx->p.n_th, use_flag,
+                                                            ctx->partial);
     else
         prep_fields_kernel<double><<<NPARTIAL, 256, 0, st>>>((const double *)d_nH, (const double *)d_xHI, ctx->absorber,
-                                                             ctx->ncell, ctx->p.n_th, use_flag, ctx->partial);
+                                                             ctx->g.nx, ctx->g.ny, ctx->g.nz, ctx->p.n_th, use_flag,
+                                                             ctx->partial);
     sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 0);
     CU(cudaGetLastError());
     ctx->d_nH = d_nH;
@@ -456,7 +483,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     sum_flux_kernel<<<1, 256, 0, st>>>(s.L2[0], ctx->n_cat, ctx->scalars + 2);
     CU(cudaEventRecord(ctx->ev[1], st));
     // ---- ray loop ----
-    CU(cudaMemsetAsync(d_gamma, 0, ctx->ncell * sizeof(double), st));
+    CU(cudaMemsetAsync(ctx->acc, 0, ctx->pcell * sizeof(double), st));
     CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
     memset(ctx->h_ls, 0, sizeof(LoopState));
     ctx->h_ls->n_cat = ctx->n_cat;
@@ -465,7 +492,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     MarchArgs a;
     memset(&a, 0, sizeof a);
     a.absorber = ctx->absorber;
-    a.acc = d_gamma;
+    a.acc = ctx->acc;
     a.cat_cell = s.cell[0];
     a.cat_L = s.L2[0];
     a.pool = ctx->pool;
@@ -473,6 +500,8 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     a.ds = ctx->ds;
     a.nx = ctx->g.nx; a.ny = ctx->g.ny; a.nz = ctx->g.nz;
     a.level_max = ctx->p.level_max;
+    a.px = ctx->g.nx + 2;
+    a.pxy = (long long)(ctx->g.nx + 2) * (ctx->g.ny + 2);
     a.sdx = ctx->p.sigma_cm2 * ctx->g.dx_cm;
     a.tau_max = ctx->p.tau_max;
     for (int l = 0; l < MAXLEV; ++l) { a.r2_split[l] = ctx->r2_split[l]; a.K[l] = ctx->K[l]; }
@@ -494,10 +523,10 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
             switch (gt) {
-                case 0: launch_march<0>(a, ctx->march_blocks, st); break;
-                case 1: launch_march<1>(a, ctx->march_blocks, st); break;
-                case 4: launch_march<4>(a, ctx->march_blocks, st); break;
-                default: launch_march<3>(a, ctx->march_blocks, st); break;
+                case 0: launch_march<0>(a, ctx->idx64, ctx->march_blocks, st); break;
+                case 1: launch_march<1>(a, ctx->idx64, ctx->march_blocks, st); break;
+                case 4: launch_march<4>(a, ctx->idx64, ctx->march_blocks, st); break;
+                default: launch_march<3>(a, ctx->idx64, ctx->march_blocks, st); break;
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch + 1], st));
             ++n_launch;
@@ -511,8 +540,8 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     CU(cudaEventRecord(ctx->ev[2], st));
     // ---- finalise ----
     const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
-    finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->absorber, ctx->ncell, V, ctx->p.e_excess_erg,
-                                              ctx->partial);
+    finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->acc, ctx->absorber, ctx->g.nx, ctx->g.ny, ctx->g.nz, V,
+                                              ctx->p.e_excess_erg, ctx->partial);
     sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
     CU(cudaEventRecord(ctx->ev[3], st));
     CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));
@@ -523,7 +552,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
         memset(hs, 0, sizeof *hs);
         const DevStats &d = *ctx->h_ds;
         for (int l = 0; l < MAXLEV; ++l) {
-            hs->spawned[l] = d.spawned[l]; hs->split[l] = d.split[l]; hs->killed_tau[l] = d.killed_tau[l];
+            hs->spawned[l] = d.spawned[l] - d.holes[l]; hs->split[l] = d.split[l]; hs->killed_tau[l] = d.killed_tau[l];
             hs->exited[l] = d.exited[l]; hs->killed_lmax[l] = d.killed_lmax[l];
         }
         hs->segments = d.segments;

@@ -31,27 +31,35 @@ struct LoopState {
     int level;
     int done;
     int overflow;
-    int pad_;
+    int seg_round;                       // segments marched between two refills of idle lanes
     unsigned long long iterations, peak_pool;
+    unsigned long long fetch;            // next unclaimed ray of the current batch (chunks of FETCH_CHUNK)
 };
 
 struct DevStats {
     unsigned long long spawned[MAXLEV], split[MAXLEV], killed_tau[MAXLEV], exited[MAXLEV], killed_lmax[MAXLEV];
+    unsigned long long holes[MAXLEV];   // filler slots popped at level l (slab padding; not rays)
     unsigned long long segments, zero_len;
     double escaped, residual, lost;
     double absorbed;                     // finalise: sum over cells
     double emitted;
 };
 
+constexpr uint64_t KEY_HOLE = ~0ull;     // filler slot (end of a warp's child slab)
+constexpr int CHILD_SLAB = 128;          // child slots a warp reserves per atomic (>= 4 * 32)
+constexpr int FETCH_CHUNK = 128;         // rays a warp claims per atomic
+
 struct MarchArgs {
-    const double *absorber;              // |a| = n_H x_HI; sign bit set where n_H < n_th (Eq. 7-8 flag)
-    double *acc;                         // photons absorbed per cell (becomes Gamma in finalise)
+    const double *absorber;              // PADDED grid (nx+2)(ny+2)(nz+2): |a| = n_H x_HI; sign bit set where
+                                         // n_H < n_th (Eq. 7-8 flag); halo = -inf (outside the box)
+    double *acc;                         // PADDED: photons absorbed per cell
     const int4 *cat_cell;                // (i, j, k, 0) per catalogue source
     const double *cat_L;
     RayPool pool;
     LoopState *ls;
     DevStats *ds;
     int nx, ny, nz, level_max;
+    long long px, pxy;                   // padded strides: px = nx+2, pxy = (nx+2)(ny+2)
     double sdx;                          // sigma * dx: optical depth per unit absorber per cell length
     double tau_max;
     double r2_split[MAXLEV];             // Eq. 4: split when s^2 > 3 4^l / (pi N_min)
