@@ -7,10 +7,10 @@
 // (BASELINE.json configs; reading R20) or the split criterion Eq. 4, in which case the
 // four children are pushed on the stack of level+1.
 //
-// Kernel shape (sm_100a, issue-bound rather than HBM-bound, see profiles/): persistent warps.  A warp claims
-// chunks of rays, initialises 32 at a time with all lanes active (HEALPix direction, start cell), parks
-// them in a shared-memory queue, and its lanes pop a new ray whenever theirs ends, so ray-length tails do
-// not idle lanes.  The grids are padded by one halo cell holding -inf: leaving the box is "the absorber I
+// Kernel shape (sm_100a, latency- and issue-bound rather than HBM-bound, see profiles/): persistent warps.
+// A warp claims chunks of rays; whenever enough of its lanes are idle they take new rays straight from the
+// batch (HEALPix direction, start cell), so ray-length tails do not idle lanes, and no shared memory is
+// taken from the L1 that serves the field gathers.  The grids are padded by one halo cell holding -inf: leaving the box is "the absorber I
 // just loaded is -inf", a neighbour outside the box is never eligible, and no cell coordinates are tracked.
 //
 // Everything that steers control flow follows DESIGN.md's DEC list literally; this translation unit is
@@ -21,9 +21,9 @@
 
 namespace nyxrt {
 
-constexpr int MARCH_THREADS = 256;
+constexpr int MARCH_THREADS = 128;
 constexpr int MARCH_WARPS = MARCH_THREADS / 32;
-constexpr int QCAP = 64;                 // queue entries per warp (power of two, >= 2 * 32)
+constexpr int MARCH_MIN_BLOCKS = 5;      // 20 warps per SM at <= 96 registers, no spills (checked with -Xptxas -v)
 
 // ---------------------------------------------------------------------------------------------------
 // Scheduler: one thread decides what the next emit + march launches do.
@@ -72,7 +72,8 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->level = pick;
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
-    ls->seg_round = pick < 2 ? 1 : (pick < 4 ? 2 : 4);
+    ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 1 : (pick < 4 ? 2 : 4));
+    ls->refill_min = ls->tune_refill_min > 0 ? ls->tune_refill_min : (pick < 4 ? 16 : 8);
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
@@ -95,10 +96,29 @@ __global__ void emit_kernel(const LoopState *ls, RayPool pool, const double *cat
 
 // ---------------------------------------------------------------------------------------------------
 // exp(-x) and 1 - exp(-x) for x >= 0 in one pass (not DEC: the tolerance is 1e-9).
-// x = k ln2 + r, |r| <= ln2/2; e^-r - 1 by its Taylor series through r^13 (remainder < 1e-17 relative);
-// left = 2^-k (1 + p), gone = 1 - left = -(2^-k p + (2^-k - 1)) with both terms exact up to one rounding,
-// so thin cells (k = 0, gone = -p = x - x^2/2 + ...) keep full relative accuracy where 1 - exp(-x) would not.
+// Thin cells (x < 2^-7, the ionised phase): e^-x - 1 = p by its Taylor series through x^7 (remainder
+// < 5e-20 relative), gone = -p keeps full relative accuracy where 1 - exp(-x) would not.
+// Otherwise x = k ln2 + r, |r| <= ln2/2; e^-r - 1 by its Taylor series through r^13 (remainder < 1e-17
+// relative); left = 2^-k (1 + p), gone = 1 - left = -(2^-k p + (2^-k - 1)), both terms exact up to one
+// rounding.  Coefficients sit in constant memory so that they are operands, not re-materialised immediates.
+__constant__ double EXPC[12] = {1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0,
+                                1.0 / 362880.0,     1.0 / 40320.0,     1.0 / 5040.0,     1.0 / 720.0,
+                                1.0 / 120.0,        1.0 / 24.0,        1.0 / 6.0,        0.5};
+
 __device__ __forceinline__ void absorb_fraction(double x, double &gone, double &left) {
+    const double t = -x;
+    if (x < 0.0078125) {
+        double q = EXPC[6];
+        q = fma(q, t, EXPC[7]);
+        q = fma(q, t, EXPC[8]);
+        q = fma(q, t, EXPC[9]);
+        q = fma(q, t, EXPC[10]);
+        q = fma(q, t, EXPC[11]);
+        const double p = fma(t * t, q, t);                       // e^t - 1
+        gone = -p;
+        left = 1.0 + p;
+        return;
+    }
     if (x > 690.0) { gone = 1.0; left = 0.0; return; }
     const double MAGIC = 6755399441055744.0;                     // 1.5 * 2^52: round to nearest integer
     const double kd_m = fma(x, 1.4426950408889634, MAGIC);
@@ -106,20 +126,11 @@ __device__ __forceinline__ void absorb_fraction(double x, double &gone, double &
     const double kd = kd_m - MAGIC;
     double r = fma(kd, -6.93147180369123816490e-01, x);          // ln2 hi
     r = fma(kd, -1.90821492927058770002e-10, r);                 // ln2 lo
-    const double t = -r;
-    double q = 1.0 / 6227020800.0;                               // 1/13!
-    q = fma(q, t, 1.0 / 479001600.0);
-    q = fma(q, t, 1.0 / 39916800.0);
-    q = fma(q, t, 1.0 / 3628800.0);
-    q = fma(q, t, 1.0 / 362880.0);
-    q = fma(q, t, 1.0 / 40320.0);
-    q = fma(q, t, 1.0 / 5040.0);
-    q = fma(q, t, 1.0 / 720.0);
-    q = fma(q, t, 1.0 / 120.0);
-    q = fma(q, t, 1.0 / 24.0);
-    q = fma(q, t, 1.0 / 6.0);
-    q = fma(q, t, 0.5);
-    const double p = fma(t * t, q, t);                           // e^t - 1
+    const double u = -r;
+    double q = EXPC[0];
+#pragma unroll
+    for (int i = 1; i < 12; ++i) q = fma(q, u, EXPC[i]);
+    const double p = fma(u * u, q, u);                           // e^u - 1
     const double sc = __hiloint2double((1023 - k) << 20, 0);     // 2^-k
     left = fma(sc, p, sc);
     gone = -fma(sc, p, sc - 1.0);
@@ -139,55 +150,52 @@ __device__ __forceinline__ double div_fast(double a, double b) {
 
 enum { OUT_NONE = 0, OUT_SPLIT = 1, OUT_KILL_TAU = 2, OUT_EXIT = 3, OUT_KILL_LMAX = 4 };
 
-// shared-memory queue of initialised rays, one per warp, structure of arrays
-struct WarpQueue {
-    unsigned long long key[QCAP];
-    double s[QCAP], tau[QCAP], N[QCAP];
-    double d[3][QCAP], inv[3][QCAP], od[3][QCAP];
-    long long c[QCAP];
-    int up[QCAP];
+// per-thread scratch that is touched only when a ray is born or retires (kept out of registers)
+struct ThreadScratch {
+    unsigned long long key[MARCH_THREADS];
+    double esc[MARCH_THREADS], res[MARCH_THREADS];
 };
 
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
 template <int GEOM, typename IDX>
-__global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_constant__ MarchArgs A) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(const __grid_constant__ MarchArgs A) {
+    __shared__ ThreadScratch T;
     const LoopState *ls = A.ls;
     const long long batch = ls->batch;
     if (batch == 0) return;
     const int level = ls->level;
     const int seg_round = ls->seg_round;
+    const int refill_min = ls->refill_min;
     const long long begin = ls->begin;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    WarpQueue &Q = reinterpret_cast<WarpQueue *>(smem_raw)[threadIdx.x >> 5];
     const double r2s = A.r2_split[level], Kl = A.K[level], Kh = 0.5 * A.K[level];
     const double tau_max = A.tau_max, sdx = A.sdx;
     const IDX sy = (IDX)A.px, sz = (IDX)A.pxy;
     const double *__restrict__ absorber = A.absorber;
     double *__restrict__ acc = A.acc;
 
+    T.esc[threadIdx.x] = 0.0;
+    T.res[threadIdx.x] = 0.0;
     unsigned int n_seg = 0, n_zero = 0;
     unsigned int n_split = 0, n_ktau = 0, n_exit = 0, n_klmax = 0, n_hole = 0;   // lane 0 holds warp totals
-    double esc = 0.0, res = 0.0, lost = 0.0;
+    double lost = 0.0;
 
     // warp-uniform bookkeeping
-    int qhead = 0, qcount = 0;
     long long chunk_pos = 0, chunk_end = 0;
     bool exhausted = false;
     long long slab_pos = 0, slab_end = 0;          // child slots reserved on the stack of level+1
 
     // per-lane ray state
     bool has = false;
-    unsigned long long key = 0;
     double s = 0.0, tau = 0.0, N = 0.0;
     double d0 = 0, d1 = 0, d2 = 0, inv0 = 0, inv1 = 0, inv2 = 0, od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
     double a_raw = 0.0;
-    IDX c = 0, cs0 = 0, cs1 = 0, cs2 = 0;
+    IDX c = 0;
     int up = 0;
 
     // retire rays whose outcome is known (all lanes call it; outcome NONE = nothing to do)
-    auto retire = [&](int outcome, unsigned long long rkey, double rs, double rtau, double rN) {
+    auto retire = [&](int outcome, double rs, double rtau, double rN) {
         const unsigned m_any = __ballot_sync(0xffffffffu, outcome != OUT_NONE);
         if (m_any == 0) return;
         const unsigned m_split = __ballot_sync(0xffffffffu, outcome == OUT_SPLIT);
@@ -197,8 +205,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_co
         if (lane == 0) {
             n_split += __popc(m_split); n_ktau += __popc(m_ktau); n_exit += __popc(m_exit); n_klmax += __popc(m_klmax);
         }
-        if (outcome == OUT_EXIT) esc += rN;
-        else if (outcome == OUT_KILL_TAU || outcome == OUT_KILL_LMAX) res += rN;
+        if (outcome == OUT_EXIT) T.esc[threadIdx.x] += rN;
+        else if (outcome == OUT_KILL_TAU || outcome == OUT_KILL_LMAX) T.res[threadIdx.x] += rN;
         if (m_split) {
             const int need = 4 * __popc(m_split);
             if (slab_pos + need > slab_end) {
@@ -217,6 +225,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_co
                 slab_end = base + CHILD_SLAB;
             }
             if (outcome == OUT_SPLIT) {
+                const unsigned long long rkey = T.key[threadIdx.x];
                 const long long w = A.pool.off[level + 1] + slab_pos + 4 * __popc(m_split & lt);
                 const uint32_t src = key_src(rkey), p4 = 4u * key_pix(rkey);
                 const double Nc = rN * 0.25;                                     // L shared evenly
@@ -233,96 +242,66 @@ __global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_co
     };
 
     for (;;) {
-        // ---- top up the queue: 32 rays at a time, all lanes active --------------------------------
-        while (qcount <= QCAP - 32 && !exhausted) {
+        // ---- refill: idle lanes take new rays straight from the batch -----------------------------------
+        // (no staging queue: a far-field ray lives for hundreds of cells, so initialising with a partly
+        // idle warp costs little, and the shared memory stays with the L1)
+        const unsigned m_idle = __ballot_sync(0xffffffffu, !has);
+        const int n_idle = __popc(m_idle);
+        if (!exhausted && (n_idle >= refill_min || n_idle == 32)) {
             if (chunk_pos >= chunk_end) {
                 unsigned long long f = 0;
                 if (lane == 0) f = atomicAdd((unsigned long long *)&A.ls->fetch, (unsigned long long)FETCH_CHUNK);
                 f = __shfl_sync(0xffffffffu, f, 0);
-                if ((long long)f >= batch) { exhausted = true; break; }
+                if ((long long)f >= batch) { exhausted = true; continue; }
                 chunk_pos = (long long)f;
                 chunk_end = chunk_pos + FETCH_CHUNK < batch ? chunk_pos + FETCH_CHUNK : batch;
             }
-            const long long r = chunk_pos + lane;
-            chunk_pos += 32;
+            const long long avail = chunk_end - chunk_pos;
+            const int take = n_idle < avail ? n_idle : (int)avail;
+            const int rank = __popc(m_idle & lt);
+            const bool mine = !has && rank < take;
+            const long long r = begin + chunk_pos + rank;
+            chunk_pos += take;
             int outcome = OUT_NONE;
-            bool march = false;
             unsigned long long ikey = KEY_HOLE;
-            double is = 0.0, itau = 0.0, iN = 0.0;
-            if (r < chunk_end) ikey = A.pool.key[begin + r];
+            if (mine) ikey = A.pool.key[r];
             const bool real = ikey != KEY_HOLE;
-            const unsigned m_hole = __ballot_sync(0xffffffffu, r < chunk_end && !real);
+            const unsigned m_hole = __ballot_sync(0xffffffffu, mine && !real);
             if (lane == 0) n_hole += __popc(m_hole);
-            double e0 = 0, e1 = 0, e2 = 0, i0 = 0, i1 = 0, i2 = 0, f0 = 0, f1 = 0, f2 = 0;
-            long long ic = 0;
-            int iup = 0;
             if (real) {
-                is = A.pool.s[begin + r];
-                itau = A.pool.tau[begin + r];
-                iN = A.pool.N[begin + r];
+                s = A.pool.s[r];
+                tau = A.pool.tau[r];
+                N = A.pool.N[r];
+                T.key[threadIdx.x] = ikey;
                 const int4 sc = A.cat_cell[key_src(ikey)];
-                pix2dir(level, key_pix(ikey), e0, e1, e2);
+                pix2dir(level, key_pix(ikey), d0, d1, d2);
                 // O4: start-of-life cell, source-relative (source at its cell centre)
                 double q;
-                q = fma(is, e0, 0.5); f0 = floor(q); if (q == f0 && e0 < 0.0) f0 -= 1.0;
-                q = fma(is, e1, 0.5); f1 = floor(q); if (q == f1 && e1 < 0.0) f1 -= 1.0;
-                q = fma(is, e2, 0.5); f2 = floor(q); if (q == f2 && e2 < 0.0) f2 -= 1.0;
-                iup = (e0 > 0.0 ? 1 : 0) | (e1 > 0.0 ? 2 : 0) | (e2 > 0.0 ? 4 : 0);
-                i0 = (e0 == 0.0) ? -CUDART_INF : 1.0 / e0;                   // with od + (-0.5): s_x = +inf
-                i1 = (e1 == 0.0) ? -CUDART_INF : 1.0 / e1;
-                i2 = (e2 == 0.0) ? -CUDART_INF : 1.0 / e2;
-                const long long ci = sc.x + (long long)f0, cj = sc.y + (long long)f1, ck = sc.z + (long long)f2;
+                q = fma(s, d0, 0.5); od0 = floor(q); if (q == od0 && d0 < 0.0) od0 -= 1.0;
+                q = fma(s, d1, 0.5); od1 = floor(q); if (q == od1 && d1 < 0.0) od1 -= 1.0;
+                q = fma(s, d2, 0.5); od2 = floor(q); if (q == od2 && d2 < 0.0) od2 -= 1.0;
+                up = (d0 > 0.0 ? 1 : 0) | (d1 > 0.0 ? 2 : 0) | (d2 > 0.0 ? 4 : 0);
+                inv0 = (d0 == 0.0) ? -CUDART_INF : 1.0 / d0;                   // with od + (-0.5): s_x = +inf
+                inv1 = (d1 == 0.0) ? -CUDART_INF : 1.0 / d1;
+                inv2 = (d2 == 0.0) ? -CUDART_INF : 1.0 / d2;
+                const long long ci = sc.x + (long long)od0, cj = sc.y + (long long)od1, ck = sc.z + (long long)od2;
                 if (ci < 0 || ci >= A.nx || cj < 0 || cj >= A.ny || ck < 0 || ck >= A.nz) outcome = OUT_EXIT;
-                else if (itau >= tau_max) outcome = OUT_KILL_TAU;
+                else if (tau >= tau_max) outcome = OUT_KILL_TAU;
                 else if (level >= A.level_max) outcome = OUT_KILL_LMAX;
-                else if (is * is > r2s) outcome = OUT_SPLIT;
-                else { march = true; ic = ((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1); }
-            }
-            retire(outcome, ikey, is, itau, iN);
-            const unsigned mm = __ballot_sync(0xffffffffu, march);
-            if (march) {
-                const int slot = (qhead + qcount + __popc(mm & lt)) & (QCAP - 1);
-                Q.key[slot] = ikey; Q.s[slot] = is; Q.tau[slot] = itau; Q.N[slot] = iN;
-                Q.d[0][slot] = e0; Q.d[1][slot] = e1; Q.d[2][slot] = e2;
-                Q.inv[0][slot] = i0; Q.inv[1][slot] = i1; Q.inv[2][slot] = i2;
-                Q.od[0][slot] = f0; Q.od[1][slot] = f1; Q.od[2][slot] = f2;
-                Q.c[slot] = ic; Q.up[slot] = iup;
-            }
-            qcount += __popc(mm);
-            __syncwarp();
-        }
-        // ---- idle lanes pop a ray ---------------------------------------------------------------------
-        {
-            const unsigned m_need = __ballot_sync(0xffffffffu, !has);
-            if (m_need != 0 && qcount > 0) {
-                const int rank = __popc(m_need & lt);
-                if (!has && rank < qcount) {
-                    const int slot = (qhead + rank) & (QCAP - 1);
-                    key = Q.key[slot]; s = Q.s[slot]; tau = Q.tau[slot]; N = Q.N[slot];
-                    d0 = Q.d[0][slot]; d1 = Q.d[1][slot]; d2 = Q.d[2][slot];
-                    inv0 = Q.inv[0][slot]; inv1 = Q.inv[1][slot]; inv2 = Q.inv[2][slot];
-                    od0 = Q.od[0][slot]; od1 = Q.od[1][slot]; od2 = Q.od[2][slot];
-                    c = (IDX)Q.c[slot]; up = Q.up[slot];
+                else if (s * s > r2s) outcome = OUT_SPLIT;
+                else {
+                    c = (IDX)(((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1));
                     a_raw = __ldg(absorber + c);
-                    cs0 = (up & 1) ? (IDX)1 : (IDX)-1;
-                    cs1 = (up & 2) ? sy : -sy;
-                    cs2 = (up & 4) ? sz : -sz;
                     sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0;              // ((o + up) - 0.5) / d
                     sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1;
                     sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2;
                     has = true;
                 }
-                const int want = __popc(m_need);
-                const int taken = want < qcount ? want : qcount;
-                qhead = (qhead + taken) & (QCAP - 1);
-                qcount -= taken;
             }
-            __syncwarp();
-        }
-        if (__ballot_sync(0xffffffffu, has) == 0) {
-            if (exhausted && qcount == 0) break;
+            retire(outcome, s, tau, N);
             continue;
         }
+        if (n_idle == 32) break;                                                  // exhausted and nothing in flight
         // ---- march: seg_round cells per lane, then retire / refill -------------------------------------
         int outcome = OUT_NONE;
         for (int it = 0; it < seg_round; ++it) {
@@ -384,14 +363,14 @@ __global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_co
                         ++n_zero;
                     }
                     s = s_exit;
-                    if (ax == 0) { od0 += (up & 1) ? 1.0 : -1.0; c += cs0; sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0; }
-                    else if (ax == 1) { od1 += (up & 2) ? 1.0 : -1.0; c += cs1; sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1; }
-                    else { od2 += (up & 4) ? 1.0 : -1.0; c += cs2; sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2; }
+                    if (ax == 0) { od0 += (up & 1) ? 1.0 : -1.0; c += (up & 1) ? (IDX)1 : (IDX)-1; sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0; }
+                    else if (ax == 1) { od1 += (up & 2) ? 1.0 : -1.0; c += (up & 2) ? sy : -sy; sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1; }
+                    else { od2 += (up & 4) ? 1.0 : -1.0; c += (up & 4) ? sz : -sz; sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2; }
                     a_raw = __ldg(absorber + c);
                 }
             }
         }
-        retire(outcome, key, s, tau, N);
+        retire(outcome, s, tau, N);
         if (outcome != OUT_NONE) has = false;
     }
     // pad the unused tail of the last child slab
@@ -399,6 +378,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, 3) march_kernel(const __grid_co
 
     // flush per-thread / per-warp tallies
     unsigned long long seg64 = n_seg, zero64 = n_zero;
+    double esc = T.esc[threadIdx.x], res = T.res[threadIdx.x];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         seg64 += __shfl_xor_sync(0xffffffffu, seg64, o);

@@ -45,6 +45,7 @@ struct nyxrt_ctx {
     nyxrt_params p;
     char err[512];
     int sm_count, march_blocks, nlev;
+    int tune_seg_round, tune_refill_min;   // NYXRT_SEG_ROUND / NYXRT_REFILL_MIN (tuning knobs, 0 = scheduler's choice)
     long long ncell;
     // workspace
     void *ws;
@@ -188,7 +189,7 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
     return ((b.off + 255) & ~uint64_t(255));
 }
 
-constexpr size_t MARCH_SMEM = sizeof(WarpQueue) * MARCH_WARPS;
+constexpr size_t MARCH_SMEM = 0;          // the kernel's scratch is static shared memory
 
 template <int GEOM>
 void launch_march(const MarchArgs &a, bool idx64, int blocks, cudaStream_t st) {
@@ -200,11 +201,11 @@ template <int GEOM>
 cudaError_t setup_march(bool idx64, int *occ) {
     cudaError_t e;
     if (idx64) {
-        e = cudaFuncSetAttribute(march_kernel<GEOM, long long>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MARCH_SMEM);
+        e = cudaFuncSetAttribute(march_kernel<GEOM, long long>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
         if (e == cudaSuccess)
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, long long>, MARCH_THREADS, MARCH_SMEM);
     } else {
-        e = cudaFuncSetAttribute(march_kernel<GEOM, int>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MARCH_SMEM);
+        e = cudaFuncSetAttribute(march_kernel<GEOM, int>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
         if (e == cudaSuccess)
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, int>, MARCH_THREADS, MARCH_SMEM);
     }
@@ -355,6 +356,8 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     }
     ctx->sm_count = prop.multiProcessorCount;
     ctx->march_blocks = ctx->sm_count * (occ > 0 ? occ : 1);
+    if (const char *v = getenv("NYXRT_SEG_ROUND")) ctx->tune_seg_round = atoi(v);
+    if (const char *v = getenv("NYXRT_REFILL_MIN")) ctx->tune_refill_min = atoi(v);
     *out = ctx;
     return NYXRT_OK;
 }
@@ -488,6 +491,8 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     memset(ctx->h_ls, 0, sizeof(LoopState));
     ctx->h_ls->n_cat = ctx->n_cat;
     ctx->h_ls->batch_rays = ctx->batch_rays;
+    ctx->h_ls->tune_seg_round = ctx->tune_seg_round;
+    ctx->h_ls->tune_refill_min = ctx->tune_refill_min;
     CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
     MarchArgs a;
     memset(&a, 0, sizeof a);
