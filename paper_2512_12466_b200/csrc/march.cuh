@@ -23,7 +23,7 @@ namespace nyxrt {
 
 constexpr int MARCH_THREADS = 128;
 constexpr int MARCH_WARPS = MARCH_THREADS / 32;
-constexpr int MARCH_MIN_BLOCKS = 5;      // 20 warps per SM at <= 96 registers, no spills (checked with -Xptxas -v)
+constexpr int MARCH_MIN_BLOCKS = 4;      // 16 warps per SM at <= 128 registers, no spills (checked with -Xptxas -v)
 
 // ---------------------------------------------------------------------------------------------------
 // Scheduler: one thread decides what the next emit + march launches do.
@@ -105,7 +105,8 @@ __constant__ double EXPC[12] = {1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 399
                                 1.0 / 362880.0,     1.0 / 40320.0,     1.0 / 5040.0,     1.0 / 720.0,
                                 1.0 / 120.0,        1.0 / 24.0,        1.0 / 6.0,        0.5};
 
-__device__ __forceinline__ void absorb_fraction(double x, double &gone, double &left) {
+// Returns pm = e^-x - 1 (<= 0: minus the absorbed fraction) and left = e^-x.
+__device__ __forceinline__ void absorb_fraction(double x, double &pm, double &left) {
     const double t = -x;
     if (x < 0.0078125) {
         double q = EXPC[6];
@@ -114,12 +115,11 @@ __device__ __forceinline__ void absorb_fraction(double x, double &gone, double &
         q = fma(q, t, EXPC[9]);
         q = fma(q, t, EXPC[10]);
         q = fma(q, t, EXPC[11]);
-        const double p = fma(t * t, q, t);                       // e^t - 1
-        gone = -p;
-        left = 1.0 + p;
+        pm = fma(t * t, q, t);                                   // e^t - 1
+        left = 1.0 + pm;
         return;
     }
-    if (x > 690.0) { gone = 1.0; left = 0.0; return; }
+    if (x > 690.0) { pm = -1.0; left = 0.0; return; }
     const double MAGIC = 6755399441055744.0;                     // 1.5 * 2^52: round to nearest integer
     const double kd_m = fma(x, 1.4426950408889634, MAGIC);
     const int k = __double2loint(kd_m);                          // 0 .. 996
@@ -133,19 +133,27 @@ __device__ __forceinline__ void absorb_fraction(double x, double &gone, double &
     const double p = fma(u * u, q, u);                           // e^u - 1
     const double sc = __hiloint2double((1023 - k) << 20, 0);     // 2^-k
     left = fma(sc, p, sc);
-    gone = -fma(sc, p, sc - 1.0);
+    pm = fma(sc, p, sc - 1.0);
 }
 
-// a / b to ~1 ulp without the IEEE slow path (not DEC: only scales a deposit); b is a positive normal number
+// a / b to a few ulp without the IEEE slow path (not DEC: only scales a deposit); b is a positive normal
+// number.  The hardware seed is good to ~2^-20; one Newton step squares that and the residual correction of
+// the quotient squares it again, so the result is rounding-limited.
 __device__ __forceinline__ double div_fast(double a, double b) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
-    double e = fma(-b, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-b, y, 1.0);
+    const double e = fma(-b, y, 1.0);
     y = fma(y, e, y);
     const double qv = a * y;
     return fma(fma(-b, qv, a), y, qv);
+}
+
+// +-1.0 and +-0.5 with the sign of x (x = 1/d: the direction of travel along one axis)
+__device__ __forceinline__ double signed_one(double x) {
+    return __hiloint2double((__double2hiint(x) & 0x80000000) | 0x3ff00000, 0);
+}
+__device__ __forceinline__ double signed_half(double x) {
+    return __hiloint2double((__double2hiint(x) & 0x80000000) | 0x3fe00000, 0);
 }
 
 enum { OUT_NONE = 0, OUT_SPLIT = 1, OUT_KILL_TAU = 2, OUT_EXIT = 3, OUT_KILL_LMAX = 4 };
@@ -154,6 +162,16 @@ enum { OUT_NONE = 0, OUT_SPLIT = 1, OUT_KILL_TAU = 2, OUT_EXIT = 3, OUT_KILL_LMA
 struct ThreadScratch {
     unsigned long long key[MARCH_THREADS];
     double esc[MARCH_THREADS], res[MARCH_THREADS];
+};
+
+// One ray-cell segment, described by the geometry stage and consumed by the physics stage one iteration
+// later (so that its two absorber gathers have a whole iteration to arrive).
+template <typename IDX>
+struct SegDesc {
+    double a_c, a_n;      // absorber of the cell (sign = Eq. 7-8 flag, -inf = outside the box) and of the neighbour
+    double ds, s_m, de;   // length, midpoint distance, D_edge
+    IDX c, cq;            // cell and neighbour across the nearest face (cq == c: no neighbour deposit)
+    bool split;           // the cell's entry distance meets Eq. 4: the ray splits here instead of marching
 };
 
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
@@ -186,13 +204,110 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     bool exhausted = false;
     long long slab_pos = 0, slab_end = 0;          // child slots reserved on the stack of level+1
 
-    // per-lane ray state
+    // per-lane ray state.  The DDA (s, od, sx, c) runs ONE CELL AHEAD of the physics: it describes the next
+    // cell to be traversed, while SA / SB hold the segment whose absorber loads are in flight.
     bool has = false;
     double s = 0.0, tau = 0.0, N = 0.0;
     double d0 = 0, d1 = 0, d2 = 0, inv0 = 0, inv1 = 0, inv2 = 0, od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
-    double a_raw = 0.0;
-    IDX c = 0;
-    int up = 0;
+    IDX c = 0, cst0 = 0, cst1 = 0, cst2 = 0;       // cell (padded linear index) and its signed step per axis
+    SegDesc<IDX> SA, SB;
+    SA.split = SB.split = false;
+
+    // G stage: describe the cell the DDA stands in (everything here is geometry: no loaded value is needed),
+    // issue its absorber loads, and advance the DDA to the next cell.  A cell that meets the split criterion
+    // (Eq. 4, tested on the entry distance s) is only flagged: the DDA stays put, so that the children
+    // inherit s, and only the cell's own absorber is fetched (the box-exit test comes first).
+    auto describe = [&](SegDesc<IDX> &D) {
+        D.c = c;
+        D.cq = c;
+        D.a_c = __ldg(absorber + c);
+        D.a_n = 0.0;
+        D.split = s * s > r2s;
+        if (D.split) return;
+        double s_exit = sx0; int ax = 0;
+        if (sx1 < s_exit) { s_exit = sx1; ax = 1; }
+        if (sx2 < s_exit) { s_exit = sx2; ax = 2; }                               // first minimum, order x, y, z
+        double ds = s_exit - s;
+        if (!(ds > 0.0)) ds = 0.0;
+        D.ds = ds;
+        if (GEOM != 0) {
+            const double s_m = fma(0.5, ds, s);                                   // = s + 0.5 ds (0.5 ds is exact)
+            D.s_m = s_m;
+            double m0 = fma(s_m, d0, 0.5) - od0;
+            double m1 = fma(s_m, d1, 0.5) - od1;
+            double m2 = fma(s_m, d2, 0.5) - od2;
+            // nearest face, first minimum in the order x-, x+, y-, y+, z-, z+ (ties inside an axis go to the
+            // minus side, ties between axes to the earlier axis: the same choice as six sequential tests)
+            double t0 = 1.0 - m0, t1 = 1.0 - m1, t2 = 1.0 - m2;
+            double h0 = m0; IDX f0 = (IDX)-1;
+            if (t0 < h0) { h0 = t0; f0 = (IDX)1; }
+            double h1 = m1; IDX f1 = -sy;
+            if (t1 < h1) { h1 = t1; f1 = sy; }
+            double h2 = m2; IDX f2 = -sz;
+            if (t2 < h2) { h2 = t2; f2 = sz; }
+            double de = h0; IDX off = f0;
+            if (h1 < de) { de = h1; off = f1; }
+            if (h2 < de) { de = h2; off = f2; }
+            if (de < 0.0) {
+                // rounding put the midpoint a hair outside the cell: redo with the clamp to [0, 1] of the
+                // DEC list (rare; when every m is inside [0, 1] the clamp changes nothing)
+                m0 = m0 < 0.0 ? 0.0 : (m0 > 1.0 ? 1.0 : m0);
+                m1 = m1 < 0.0 ? 0.0 : (m1 > 1.0 ? 1.0 : m1);
+                m2 = m2 < 0.0 ? 0.0 : (m2 > 1.0 ? 1.0 : m2);
+                de = m0; off = (IDX)-1;
+                double t = 1.0 - m0; if (t < de) { de = t; off = (IDX)1; }
+                if (m1 < de) { de = m1; off = -sy; }
+                t = 1.0 - m1; if (t < de) { de = t; off = sy; }
+                if (m2 < de) { de = m2; off = -sz; }
+                t = 1.0 - m2; if (t < de) { de = t; off = sz; }
+            }
+            D.de = de;
+            if (de < s_m * Kh && ds > 0.0) {                                      // D_edge < L_pix / 2  (Eq. 5 / 7)
+                D.cq = c + off;                                                   // cq != c marks "eligible"
+                if (GEOM == 3) D.a_n = __ldg(absorber + D.cq);
+            }
+        }
+        // advance one cell (DEC: s = s_exit; s_a = ((o_a + [d_a > 0]) - 0.5) / d_a)
+        s = s_exit;
+        if (ax == 0) { od0 += signed_one(inv0); sx0 = (od0 + signed_half(inv0)) * inv0; }
+        if (ax == 1) { od1 += signed_one(inv1); sx1 = (od1 + signed_half(inv1)) * inv1; }
+        if (ax == 2) { od2 += signed_one(inv2); sx2 = (od2 + signed_half(inv2)) * inv2; }
+        c += ax == 0 ? cst0 : (ax == 1 ? cst1 : cst2);
+    };
+
+    // P stage: the tests in the oracle's order (box exit, filter, split), then the segment's absorption and
+    // its deposit (Eq. 1-2, 5-8).  Returns the ray's outcome.
+    auto physics = [&](const SegDesc<IDX> &D) -> int {
+        if (D.a_c == -CUDART_INF) return OUT_EXIT;
+        if (tau >= tau_max) return OUT_KILL_TAU;
+        if (D.split) return OUT_SPLIT;
+        if (D.ds > 0.0) {
+            ++n_seg;
+            const double a_c = fabs(D.a_c);
+            const double dtau = (a_c * sdx) * D.ds;
+            double pm, left;
+            absorb_fraction(dtau, pm, left);
+            const double dN = N * (-pm);
+            if (dN > 0.0) {
+                double fc = 1.0;
+                if (GEOM == 3) {
+                    if (D.a_n > 0.0) {                                            // in the box, absorber > 0, n_H >= n_th
+                        fc = 0.5 + div_fast(D.de, D.s_m * Kl);
+                        atomicAdd(acc + D.cq, (1.0 - fc) * dN);
+                    }
+                } else if (GEOM == 1 || GEOM == 4) {
+                    if (D.cq != D.c) { fc = 0.5 + div_fast(D.de, D.s_m * Kl); if (GEOM == 4) fc = fc * fc; }
+                    lost += (1.0 - fc) * dN;
+                }
+                atomicAdd(acc + D.c, fc * dN);
+            }
+            N = N * left;
+            tau = tau + dtau;
+        } else {
+            ++n_zero;
+        }
+        return OUT_NONE;
+    };
 
     // retire rays whose outcome is known (all lanes call it; outcome NONE = nothing to do)
     auto retire = [&](int outcome, double rs, double rtau, double rN) {
@@ -208,25 +323,27 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         if (outcome == OUT_EXIT) T.esc[threadIdx.x] += rN;
         else if (outcome == OUT_KILL_TAU || outcome == OUT_KILL_LMAX) T.res[threadIdx.x] += rN;
         if (m_split) {
+            // children go to the warp's slab on the stack of level+1; when the slab cannot hold them all, the
+            // first `rem` slots (a multiple of 4) finish the old slab and the rest start a new one: no slot is
+            // wasted, so B marched rays push at most 4B children (+ one partly used slab per warp per launch)
             const int need = 4 * __popc(m_split);
-            if (slab_pos + need > slab_end) {
-                // pad the rest of the old slab with holes, reserve a new one
-                for (long long h = slab_pos + lane; h < slab_end; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
-                long long base = 0;
+            const long long rem = slab_end - slab_pos;
+            long long base = 0;
+            if (need > rem) {
                 if (lane == 0) base = (long long)atomicAdd((unsigned long long *)&A.ls->count[level + 1],
                                                            (unsigned long long)CHILD_SLAB);
                 base = __shfl_sync(0xffffffffu, base, 0);
                 if (base + CHILD_SLAB > A.pool.cap[level + 1]) {
                     if (lane == 0) A.ls->overflow = 1;
+                    for (long long h = slab_pos + lane; h < slab_end; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
                     slab_pos = slab_end = 0;
                     return;
                 }
-                slab_pos = base;
-                slab_end = base + CHILD_SLAB;
             }
             if (outcome == OUT_SPLIT) {
                 const unsigned long long rkey = T.key[threadIdx.x];
-                const long long w = A.pool.off[level + 1] + slab_pos + 4 * __popc(m_split & lt);
+                const long long lo = 4 * __popc(m_split & lt);
+                const long long w = A.pool.off[level + 1] + (lo < rem ? slab_pos + lo : base + (lo - rem));
                 const uint32_t src = key_src(rkey), p4 = 4u * key_pix(rkey);
                 const double Nc = rN * 0.25;                                     // L shared evenly
 #pragma unroll
@@ -237,7 +354,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                     A.pool.N[w + k] = Nc;
                 }
             }
-            slab_pos += need;
+            if (need > rem) { slab_pos = base + (need - rem); slab_end = base + CHILD_SLAB; }
+            else slab_pos += need;
         }
     };
 
@@ -280,7 +398,6 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 q = fma(s, d0, 0.5); od0 = floor(q); if (q == od0 && d0 < 0.0) od0 -= 1.0;
                 q = fma(s, d1, 0.5); od1 = floor(q); if (q == od1 && d1 < 0.0) od1 -= 1.0;
                 q = fma(s, d2, 0.5); od2 = floor(q); if (q == od2 && d2 < 0.0) od2 -= 1.0;
-                up = (d0 > 0.0 ? 1 : 0) | (d1 > 0.0 ? 2 : 0) | (d2 > 0.0 ? 4 : 0);
                 inv0 = (d0 == 0.0) ? -CUDART_INF : 1.0 / d0;                   // with od + (-0.5): s_x = +inf
                 inv1 = (d1 == 0.0) ? -CUDART_INF : 1.0 / d1;
                 inv2 = (d2 == 0.0) ? -CUDART_INF : 1.0 / d2;
@@ -291,82 +408,31 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 else if (s * s > r2s) outcome = OUT_SPLIT;
                 else {
                     c = (IDX)(((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1));
-                    a_raw = __ldg(absorber + c);
-                    sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0;              // ((o + up) - 0.5) / d
-                    sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1;
-                    sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2;
+                    cst0 = d0 > 0.0 ? (IDX)1 : (IDX)-1;
+                    cst1 = d1 > 0.0 ? sy : -sy;
+                    cst2 = d2 > 0.0 ? sz : -sz;
+                    sx0 = (od0 + signed_half(inv0)) * inv0;                    // ((o + [d > 0]) - 0.5) / d
+                    sx1 = (od1 + signed_half(inv1)) * inv1;
+                    sx2 = (od2 + signed_half(inv2)) * inv2;
                     has = true;
+                    describe(SA);                                              // first segment: loads in flight
                 }
             }
             retire(outcome, s, tau, N);
             continue;
         }
         if (n_idle == 32) break;                                                  // exhausted and nothing in flight
-        // ---- march: seg_round cells per lane, then retire / refill -------------------------------------
+        // ---- march: seg_round/2 pairs of cells per lane, then retire / refill --------------------------
+        // Software pipeline: while the physics of one segment runs, the geometry stage has already issued
+        // the loads of the next one.  SA is the pending segment on entry and on exit of every pair.
         int outcome = OUT_NONE;
-        for (int it = 0; it < seg_round; ++it) {
+        for (int it = 0; it < seg_round; it += 2) {
             if (has && outcome == OUT_NONE) {
-                // geometry of the cell the ray is in (side-effect free, overlaps the absorber load)
-                double s_exit = sx0; int ax = 0;
-                if (sx1 < s_exit) { s_exit = sx1; ax = 1; }
-                if (sx2 < s_exit) { s_exit = sx2; ax = 2; }                       // first minimum, order x, y, z
-                double ds = s_exit - s;
-                if (!(ds > 0.0)) ds = 0.0;
-                bool elig = false;
-                double de = 0.0, s_m = 0.0, a_n = 0.0;
-                IDX cq = c;
-                if (GEOM != 0) {
-                    s_m = s + 0.5 * ds;
-                    double m0 = fma(s_m, d0, 0.5) - od0;
-                    double m1 = fma(s_m, d1, 0.5) - od1;
-                    double m2 = fma(s_m, d2, 0.5) - od2;
-                    m0 = m0 < 0.0 ? 0.0 : (m0 > 1.0 ? 1.0 : m0);
-                    m1 = m1 < 0.0 ? 0.0 : (m1 > 1.0 ? 1.0 : m1);
-                    m2 = m2 < 0.0 ? 0.0 : (m2 > 1.0 ? 1.0 : m2);
-                    de = m0; IDX off = (IDX)-1;                                   // first minimum: x-,x+,y-,y+,z-,z+
-                    double t = 1.0 - m0; if (t < de) { de = t; off = (IDX)1; }
-                    if (m1 < de) { de = m1; off = -sy; }
-                    t = 1.0 - m1; if (t < de) { de = t; off = sy; }
-                    if (m2 < de) { de = m2; off = -sz; }
-                    t = 1.0 - m2; if (t < de) { de = t; off = sz; }
-                    elig = de < s_m * Kh;                                         // D_edge < L_pix / 2  (Eq. 5 / 7)
-                    if (GEOM == 3 && elig && ds > 0.0) { cq = c + off; a_n = __ldg(absorber + cq); }
-                }
-                // order of the tests as in the oracle: box exit, filter, split, then the segment
-                if (a_raw == -CUDART_INF) { outcome = OUT_EXIT; }
-                else if (tau >= tau_max) { outcome = OUT_KILL_TAU; }
-                else if (s * s > r2s) { outcome = OUT_SPLIT; }
-                else {
-                    if (ds > 0.0) {
-                        ++n_seg;
-                        const double a_c = fabs(a_raw);
-                        const double dtau = (a_c * sdx) * ds;
-                        double gone, left;
-                        absorb_fraction(dtau, gone, left);
-                        const double dN = N * gone;
-                        if (dN > 0.0) {
-                            double fc = 1.0;
-                            if (GEOM == 3) {
-                                if (elig && a_n > 0.0) {                          // in the box, absorber > 0, n_H >= n_th
-                                    fc = 0.5 + div_fast(de, s_m * Kl);
-                                    atomicAdd(acc + cq, (1.0 - fc) * dN);
-                                }
-                            } else if (GEOM == 1 || GEOM == 4) {
-                                if (elig) { fc = 0.5 + div_fast(de, s_m * Kl); if (GEOM == 4) fc = fc * fc; }
-                                lost += (1.0 - fc) * dN;
-                            }
-                            atomicAdd(acc + c, fc * dN);
-                        }
-                        N = N * left;
-                        tau = tau + dtau;
-                    } else {
-                        ++n_zero;
-                    }
-                    s = s_exit;
-                    if (ax == 0) { od0 += (up & 1) ? 1.0 : -1.0; c += (up & 1) ? (IDX)1 : (IDX)-1; sx0 = (od0 + ((up & 1) ? 0.5 : -0.5)) * inv0; }
-                    else if (ax == 1) { od1 += (up & 2) ? 1.0 : -1.0; c += (up & 2) ? sy : -sy; sx1 = (od1 + ((up & 2) ? 0.5 : -0.5)) * inv1; }
-                    else { od2 += (up & 4) ? 1.0 : -1.0; c += (up & 4) ? sz : -sz; sx2 = (od2 + ((up & 4) ? 0.5 : -0.5)) * inv2; }
-                    a_raw = __ldg(absorber + c);
+                if (!SA.split) describe(SB);
+                outcome = physics(SA);
+                if (outcome == OUT_NONE) {
+                    if (!SB.split) describe(SA);
+                    outcome = physics(SB);
                 }
             }
         }

@@ -136,7 +136,11 @@ int effective_levels(const nyxrt_ctx *c) {
 uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, int staging) {
     Bump b{static_cast<char *>(base), 0};
     const long long n = max_sources > 0 ? max_sources : 1;
-    c->absorber = b.take<double>(c->pcell);
+    // the march's geometry stage runs one cell ahead of its box-exit test: a ray that is leaving may read
+    // (never use) up to two planes beyond the halo, so the absorber field has a guard band on both sides
+    const long long guard = 2 * ((long long)(c->g.nx + 2) * (c->g.ny + 2) + (c->g.nx + 2) + 4);
+    c->absorber = b.take<double>(c->pcell + 2 * guard);
+    if (c->absorber) c->absorber += guard;
     c->acc = b.take<double>(c->pcell);
     c->partial = b.take<double>(NPARTIAL);
     c->scalars = b.take<double>(8);

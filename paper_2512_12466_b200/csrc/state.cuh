@@ -49,7 +49,7 @@ struct DevStats {
 
 constexpr uint64_t KEY_HOLE = ~0ull;     // filler slot (end of a warp's child slab)
 constexpr int CHILD_SLAB = 128;          // child slots a warp reserves per atomic (>= 4 * 32)
-constexpr int FETCH_CHUNK = 128;         // rays a warp claims per atomic
+constexpr int FETCH_CHUNK = 32;          // rays a warp claims per atomic (small: the end of a batch is shared evenly)
 
 struct MarchArgs {
     const double *absorber;              // PADDED grid (nx+2)(ny+2)(nz+2): |a| = n_H x_HI; sign bit set where
