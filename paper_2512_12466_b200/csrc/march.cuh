@@ -174,16 +174,29 @@ struct SegDesc {
     bool split;           // the cell's entry distance meets Eq. 4: the ray splits here instead of marching
 };
 
+// Rays of the current chunk that passed their birth tests, initialised at full warp width and parked until
+// a lane falls idle (one queue of FETCH_CHUNK = 32 entries per warp; positions are never stored).
+static_assert(FETCH_CHUNK == 32, "one chunk = one ray per lane");
+template <typename IDX>
+struct RayQueue {
+    unsigned long long key[MARCH_WARPS][32];
+    double s[MARCH_WARPS][32], tau[MARCH_WARPS][32], N[MARCH_WARPS][32];
+    double d0[MARCH_WARPS][32], d1[MARCH_WARPS][32], d2[MARCH_WARPS][32];           // HEALPix direction
+    double inv0[MARCH_WARPS][32], inv1[MARCH_WARPS][32], inv2[MARCH_WARPS][32];     // 1/d (-inf where d = 0)
+    IDX c[MARCH_WARPS][32];                                                          // start cell
+};
+
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
 template <int GEOM, typename IDX>
 __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(const __grid_constant__ MarchArgs A) {
     __shared__ ThreadScratch T;
+    __shared__ RayQueue<IDX> Q;
+    const int wid = threadIdx.x >> 5;
     const LoopState *ls = A.ls;
     const long long batch = ls->batch;
     if (batch == 0) return;
     const int level = ls->level;
     const int seg_round = ls->seg_round;
-    const int refill_min = ls->refill_min;
     const long long begin = ls->begin;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
@@ -200,7 +213,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     double lost = 0.0;
 
     // warp-uniform bookkeeping
-    long long chunk_pos = 0, chunk_end = 0;
+    int qhead = 0, qn = 0;                          // the warp's parked rays: entries [qhead, qhead+qn)
     bool exhausted = false;
     long long slab_pos = 0, slab_end = 0;          // child slots reserved on the stack of level+1
 
@@ -310,7 +323,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     };
 
     // retire rays whose outcome is known (all lanes call it; outcome NONE = nothing to do)
-    auto retire = [&](int outcome, double rs, double rtau, double rN) {
+    auto retire = [&](int outcome, double rs, double rtau, double rN, unsigned long long rkey) {
         const unsigned m_any = __ballot_sync(0xffffffffu, outcome != OUT_NONE);
         if (m_any == 0) return;
         const unsigned m_split = __ballot_sync(0xffffffffu, outcome == OUT_SPLIT);
@@ -341,7 +354,6 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 }
             }
             if (outcome == OUT_SPLIT) {
-                const unsigned long long rkey = T.key[threadIdx.x];
                 const long long lo = 4 * __popc(m_split & lt);
                 const long long w = A.pool.off[level + 1] + (lo < rem ? slab_pos + lo : base + (lo - rem));
                 const uint32_t src = key_src(rkey), p4 = 4u * key_pix(rkey);
@@ -360,68 +372,99 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     };
 
     for (;;) {
-        // ---- refill: idle lanes take new rays straight from the batch -----------------------------------
-        // (no staging queue: a far-field ray lives for hundreds of cells, so initialising with a partly
-        // idle warp costs little, and the shared memory stays with the L1)
-        const unsigned m_idle = __ballot_sync(0xffffffffu, !has);
-        const int n_idle = __popc(m_idle);
-        if (!exhausted && (n_idle >= refill_min || n_idle == 32)) {
-            if (chunk_pos >= chunk_end) {
-                unsigned long long f = 0;
-                if (lane == 0) f = atomicAdd((unsigned long long *)&A.ls->fetch, (unsigned long long)FETCH_CHUNK);
-                f = __shfl_sync(0xffffffffu, f, 0);
-                if ((long long)f >= batch) { exhausted = true; continue; }
-                chunk_pos = (long long)f;
-                chunk_end = chunk_pos + FETCH_CHUNK < batch ? chunk_pos + FETCH_CHUNK : batch;
-            }
-            const long long avail = chunk_end - chunk_pos;
-            const int take = n_idle < avail ? n_idle : (int)avail;
-            const int rank = __popc(m_idle & lt);
-            const bool mine = !has && rank < take;
-            const long long r = begin + chunk_pos + rank;
-            chunk_pos += take;
+        // ---- stage: when the warp's queue is empty, ALL 32 lanes initialise the next chunk of the batch ----
+        // (HEALPix direction, 1/d, start cell, birth tests), whatever rays they are marching: the expensive
+        // set-up runs at full width, rays that end at birth (outside the box, depleted, split at once) are
+        // retired on the spot, the others are parked in shared memory until a lane falls idle.
+        if (qn == 0 && !exhausted) {
+            unsigned long long f = 0;
+            if (lane == 0) f = atomicAdd((unsigned long long *)&A.ls->fetch, (unsigned long long)FETCH_CHUNK);
+            f = __shfl_sync(0xffffffffu, f, 0);
+            if ((long long)f >= batch) { exhausted = true; continue; }
+            const bool mine = (long long)f + lane < batch;
+            const long long r = begin + (long long)f + lane;
             int outcome = OUT_NONE;
             unsigned long long ikey = KEY_HOLE;
             if (mine) ikey = A.pool.key[r];
             const bool real = ikey != KEY_HOLE;
             const unsigned m_hole = __ballot_sync(0xffffffffu, mine && !real);
             if (lane == 0) n_hole += __popc(m_hole);
+            double ts = 0.0, ttau = 0.0, tN = 0.0, e0 = 0.0, e1 = 0.0, e2 = 0.0, i0 = 0.0, i1 = 0.0, i2 = 0.0;
+            IDX tc = 0;
+            bool park = false;
             if (real) {
-                s = A.pool.s[r];
-                tau = A.pool.tau[r];
-                N = A.pool.N[r];
-                T.key[threadIdx.x] = ikey;
+                ts = A.pool.s[r];
+                ttau = A.pool.tau[r];
+                tN = A.pool.N[r];
                 const int4 sc = A.cat_cell[key_src(ikey)];
-                pix2dir(level, key_pix(ikey), d0, d1, d2);
+                pix2dir(level, key_pix(ikey), e0, e1, e2);
                 // O4: start-of-life cell, source-relative (source at its cell centre)
+                double q, o0, o1, o2;
+                q = fma(ts, e0, 0.5); o0 = floor(q); if (q == o0 && e0 < 0.0) o0 -= 1.0;
+                q = fma(ts, e1, 0.5); o1 = floor(q); if (q == o1 && e1 < 0.0) o1 -= 1.0;
+                q = fma(ts, e2, 0.5); o2 = floor(q); if (q == o2 && e2 < 0.0) o2 -= 1.0;
+                i0 = (e0 == 0.0) ? -CUDART_INF : 1.0 / e0;                     // with od + (-0.5): s_x = +inf
+                i1 = (e1 == 0.0) ? -CUDART_INF : 1.0 / e1;
+                i2 = (e2 == 0.0) ? -CUDART_INF : 1.0 / e2;
+                const long long ci = sc.x + (long long)o0, cj = sc.y + (long long)o1, ck = sc.z + (long long)o2;
+                if (ci < 0 || ci >= A.nx || cj < 0 || cj >= A.ny || ck < 0 || ck >= A.nz) outcome = OUT_EXIT;
+                else if (ttau >= tau_max) outcome = OUT_KILL_TAU;
+                else if (level >= A.level_max) outcome = OUT_KILL_LMAX;
+                else if (ts * ts > r2s) outcome = OUT_SPLIT;
+                else {
+                    tc = (IDX)(((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1));
+                    park = true;
+                }
+            }
+            const unsigned m_park = __ballot_sync(0xffffffffu, park);
+            if (park) {
+                const int e = __popc(m_park & lt);
+                Q.key[wid][e] = ikey;
+                Q.s[wid][e] = ts; Q.tau[wid][e] = ttau; Q.N[wid][e] = tN;
+                Q.d0[wid][e] = e0; Q.d1[wid][e] = e1; Q.d2[wid][e] = e2;
+                Q.inv0[wid][e] = i0; Q.inv1[wid][e] = i1; Q.inv2[wid][e] = i2;
+                Q.c[wid][e] = tc;
+            }
+            qhead = 0;
+            qn = __popc(m_park);
+            __syncwarp();
+            retire(outcome, ts, ttau, tN, ikey);
+            continue;
+        }
+        // ---- pop: idle lanes take parked rays ------------------------------------------------------------
+        const unsigned m_idle = __ballot_sync(0xffffffffu, !has);
+        if (m_idle != 0 && qn > 0) {
+            const int n_idle = __popc(m_idle);
+            const int take = n_idle < qn ? n_idle : qn;
+            const int rank = __popc(m_idle & lt);
+            if (!has && rank < take) {
+                const int e = qhead + rank;
+                T.key[threadIdx.x] = Q.key[wid][e];
+                s = Q.s[wid][e]; tau = Q.tau[wid][e]; N = Q.N[wid][e];
+                d0 = Q.d0[wid][e]; d1 = Q.d1[wid][e]; d2 = Q.d2[wid][e];
+                inv0 = Q.inv0[wid][e]; inv1 = Q.inv1[wid][e]; inv2 = Q.inv2[wid][e];
+                c = Q.c[wid][e];
                 double q;
                 q = fma(s, d0, 0.5); od0 = floor(q); if (q == od0 && d0 < 0.0) od0 -= 1.0;
                 q = fma(s, d1, 0.5); od1 = floor(q); if (q == od1 && d1 < 0.0) od1 -= 1.0;
                 q = fma(s, d2, 0.5); od2 = floor(q); if (q == od2 && d2 < 0.0) od2 -= 1.0;
-                inv0 = (d0 == 0.0) ? -CUDART_INF : 1.0 / d0;                   // with od + (-0.5): s_x = +inf
-                inv1 = (d1 == 0.0) ? -CUDART_INF : 1.0 / d1;
-                inv2 = (d2 == 0.0) ? -CUDART_INF : 1.0 / d2;
-                const long long ci = sc.x + (long long)od0, cj = sc.y + (long long)od1, ck = sc.z + (long long)od2;
-                if (ci < 0 || ci >= A.nx || cj < 0 || cj >= A.ny || ck < 0 || ck >= A.nz) outcome = OUT_EXIT;
-                else if (tau >= tau_max) outcome = OUT_KILL_TAU;
-                else if (level >= A.level_max) outcome = OUT_KILL_LMAX;
-                else if (s * s > r2s) outcome = OUT_SPLIT;
-                else {
-                    c = (IDX)(((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1));
-                    cst0 = d0 > 0.0 ? (IDX)1 : (IDX)-1;
-                    cst1 = d1 > 0.0 ? sy : -sy;
-                    cst2 = d2 > 0.0 ? sz : -sz;
-                    sx0 = (od0 + signed_half(inv0)) * inv0;                    // ((o + [d > 0]) - 0.5) / d
-                    sx1 = (od1 + signed_half(inv1)) * inv1;
-                    sx2 = (od2 + signed_half(inv2)) * inv2;
-                    has = true;
-                    describe(SA);                                              // first segment: loads in flight
-                }
+                cst0 = d0 > 0.0 ? (IDX)1 : (IDX)-1;
+                cst1 = d1 > 0.0 ? sy : -sy;
+                cst2 = d2 > 0.0 ? sz : -sz;
+                sx0 = (od0 + signed_half(inv0)) * inv0;                        // ((o + [d > 0]) - 0.5) / d
+                sx1 = (od1 + signed_half(inv1)) * inv1;
+                sx2 = (od2 + signed_half(inv2)) * inv2;
+                has = true;
+                describe(SA);                                                  // first segment: loads in flight
             }
-            retire(outcome, s, tau, N);
+            qhead += take;
+            qn -= take;
+            __syncwarp();
+        }
+        if (__ballot_sync(0xffffffffu, has) == 0) {
+            if (exhausted && qn == 0) break;                                      // nothing staged, nothing in flight
             continue;
         }
-        if (n_idle == 32) break;                                                  // exhausted and nothing in flight
         // ---- march: seg_round/2 pairs of cells per lane, then retire / refill --------------------------
         // Software pipeline: while the physics of one segment runs, the geometry stage has already issued
         // the loads of the next one.  SA is the pending segment on entry and on exit of every pair.
@@ -436,7 +479,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 }
             }
         }
-        retire(outcome, s, tau, N);
+        retire(outcome, s, tau, N, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
         if (outcome != OUT_NONE) has = false;
     }
     // pad the unused tail of the last child slab

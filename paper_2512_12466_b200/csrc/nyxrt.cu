@@ -205,11 +205,11 @@ template <int GEOM>
 cudaError_t setup_march(bool idx64, int *occ) {
     cudaError_t e;
     if (idx64) {
-        e = cudaFuncSetAttribute(march_kernel<GEOM, long long>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
+        e = cudaFuncSetAttribute(march_kernel<GEOM, long long>, cudaFuncAttributePreferredSharedMemoryCarveout, 32);
         if (e == cudaSuccess)
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, long long>, MARCH_THREADS, MARCH_SMEM);
     } else {
-        e = cudaFuncSetAttribute(march_kernel<GEOM, int>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
+        e = cudaFuncSetAttribute(march_kernel<GEOM, int>, cudaFuncAttributePreferredSharedMemoryCarveout, 32);
         if (e == cudaSuccess)
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, int>, MARCH_THREADS, MARCH_SMEM);
     }
