@@ -101,7 +101,7 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
 
 /* Size of the caller-provided device workspace.
  *   max_sources     upper bound of n in nyxrt_set_sources
- *   batch_rays      rays marched per launch B (0 = default 2^21); the ray pool holds
+ *   batch_rays      rays marched per launch B (0 = default: 2^23 from 2^29 cells, 2^22 from 2^26 cells, else 2^21); the ray pool holds
  *                   (2 + 5*(level_max+1)) * B rays of 32 bytes
  *   host_staging    non-zero: add room for the fields and outputs of nyxrt_step_host
  * Workspace layout is private.  Errors: EINVAL. */

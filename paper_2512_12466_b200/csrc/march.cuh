@@ -72,8 +72,8 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->level = pick;
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
-    ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 1 : (pick < 4 ? 2 : 4));
-    ls->refill_min = ls->tune_refill_min > 0 ? ls->tune_refill_min : (pick < 4 ? 16 : 8);
+    ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 2 : (pick < 4 ? 4 : (pick < 6 ? 8 : 16)));
+    ls->refill_min = ls->tune_refill_min > 0 ? ls->tune_refill_min : 6;
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
@@ -95,41 +95,27 @@ __global__ void emit_kernel(const LoopState *ls, RayPool pool, const double *cat
 }
 
 // ---------------------------------------------------------------------------------------------------
-// exp(-x) and 1 - exp(-x) for x >= 0 in one pass (not DEC: the tolerance is 1e-9).
-// Thin cells (x < 2^-7, the ionised phase): e^-x - 1 = p by its Taylor series through x^7 (remainder
-// < 5e-20 relative), gone = -p keeps full relative accuracy where 1 - exp(-x) would not.
-// Otherwise x = k ln2 + r, |r| <= ln2/2; e^-r - 1 by its Taylor series through r^13 (remainder < 1e-17
-// relative); left = 2^-k (1 + p), gone = 1 - left = -(2^-k p + (2^-k - 1)), both terms exact up to one
-// rounding.  Coefficients sit in constant memory so that they are operands, not re-materialised immediates.
-__constant__ double EXPC[12] = {1.0 / 6227020800.0, 1.0 / 479001600.0, 1.0 / 39916800.0, 1.0 / 3628800.0,
-                                1.0 / 362880.0,     1.0 / 40320.0,     1.0 / 5040.0,     1.0 / 720.0,
-                                1.0 / 120.0,        1.0 / 24.0,        1.0 / 6.0,        0.5};
+// pm = e^-x - 1 (minus the absorbed fraction) and left = e^-x for x >= 0 (not DEC: the tolerance is 1e-9,
+// DESIGN.md "Tolerances").  Thin cells (x < 2^-7, the ionised phase) take a short series; otherwise
+// x = k ln2 + r with |r| <= ln2/2; e^-r - 1 = u + u^2 q(u), u = -r, by its Taylor series through u^11
+// (remainder < 2e-14 relative); left = 2^-k (1 + p), pm = 2^-k p + (2^-k - 1): e^-x - 1 keeps full relative
+// accuracy where 1 - exp(-x) would not.  Coefficients sit in constant memory so that they are
+// operands, not re-materialised immediates.
+__constant__ double EXPC[10] = {1.0 / 39916800.0, 1.0 / 3628800.0, 1.0 / 362880.0, 1.0 / 40320.0, 1.0 / 5040.0,
+                                1.0 / 720.0,      1.0 / 120.0,     1.0 / 24.0,     1.0 / 6.0,     0.5};
 
-// Returns pm = e^-x - 1 (<= 0: minus the absorbed fraction) and left = e^-x.
 __device__ __forceinline__ void absorb_fraction(double x, double &pm, double &left) {
-    const double t = -x;
-    if (x < 0.0078125) {
-        double q = EXPC[6];
-        q = fma(q, t, EXPC[7]);
-        q = fma(q, t, EXPC[8]);
-        q = fma(q, t, EXPC[9]);
-        q = fma(q, t, EXPC[10]);
-        q = fma(q, t, EXPC[11]);
-        pm = fma(t * t, q, t);                                   // e^t - 1
-        left = 1.0 + pm;
-        return;
-    }
-    if (x > 690.0) { pm = -1.0; left = 0.0; return; }
+    const double xc = x < 700.0 ? x : 700.0;                     // e^-700 ~ 1e-304: nothing is left either way
     const double MAGIC = 6755399441055744.0;                     // 1.5 * 2^52: round to nearest integer
-    const double kd_m = fma(x, 1.4426950408889634, MAGIC);
-    const int k = __double2loint(kd_m);                          // 0 .. 996
+    const double kd_m = fma(xc, 1.4426950408889634, MAGIC);
+    const int k = __double2loint(kd_m);                          // 0 .. 1010
     const double kd = kd_m - MAGIC;
-    double r = fma(kd, -6.93147180369123816490e-01, x);          // ln2 hi
+    double r = fma(kd, -6.93147180369123816490e-01, xc);         // ln2 hi
     r = fma(kd, -1.90821492927058770002e-10, r);                 // ln2 lo
     const double u = -r;
     double q = EXPC[0];
 #pragma unroll
-    for (int i = 1; i < 12; ++i) q = fma(q, u, EXPC[i]);
+    for (int i = 1; i < 10; ++i) q = fma(q, u, EXPC[i]);
     const double p = fma(u * u, q, u);                           // e^u - 1
     const double sc = __hiloint2double((1023 - k) << 20, 0);     // 2^-k
     left = fma(sc, p, sc);
@@ -169,7 +155,7 @@ struct ThreadScratch {
 template <typename IDX>
 struct SegDesc {
     double a_c, a_n;      // absorber of the cell (sign = Eq. 7-8 flag, -inf = outside the box) and of the neighbour
-    double ds, s_m, de;   // length, midpoint distance, D_edge
+    double ds, fc;        // length; f_c = 1/2 + D_edge / L_pix of Eq. 5 / 7
     IDX c, cq;            // cell and neighbour across the nearest face (cq == c: no neighbour deposit)
     bool split;           // the cell's entry distance meets Eq. 4: the ray splits here instead of marching
 };
@@ -232,26 +218,27 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     // inherit s, and only the cell's own absorber is fetched (the box-exit test comes first).
     auto describe = [&](SegDesc<IDX> &D) {
         D.c = c;
-        D.cq = c;
         D.a_c = __ldg(absorber + c);
+        const bool split = s * s > r2s;
+        D.split = split;
+        D.cq = c;
         D.a_n = 0.0;
-        D.split = s * s > r2s;
-        if (D.split) return;
+        if (split) return;                                                        // rare: once per ray at most
         double s_exit = sx0; int ax = 0;
         if (sx1 < s_exit) { s_exit = sx1; ax = 1; }
         if (sx2 < s_exit) { s_exit = sx2; ax = 2; }                               // first minimum, order x, y, z
         double ds = s_exit - s;
         if (!(ds > 0.0)) ds = 0.0;
         D.ds = ds;
+        D.fc = 1.0;
         if (GEOM != 0) {
             const double s_m = fma(0.5, ds, s);                                   // = s + 0.5 ds (0.5 ds is exact)
-            D.s_m = s_m;
             double m0 = fma(s_m, d0, 0.5) - od0;
             double m1 = fma(s_m, d1, 0.5) - od1;
             double m2 = fma(s_m, d2, 0.5) - od2;
             // nearest face, first minimum in the order x-, x+, y-, y+, z-, z+ (ties inside an axis go to the
             // minus side, ties between axes to the earlier axis: the same choice as six sequential tests)
-            double t0 = 1.0 - m0, t1 = 1.0 - m1, t2 = 1.0 - m2;
+            const double t0 = 1.0 - m0, t1 = 1.0 - m1, t2 = 1.0 - m2;
             double h0 = m0; IDX f0 = (IDX)-1;
             if (t0 < h0) { h0 = t0; f0 = (IDX)1; }
             double h1 = m1; IDX f1 = -sy;
@@ -274,11 +261,13 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 if (m2 < de) { de = m2; off = -sz; }
                 t = 1.0 - m2; if (t < de) { de = t; off = sz; }
             }
-            D.de = de;
-            if (de < s_m * Kh && ds > 0.0) {                                      // D_edge < L_pix / 2  (Eq. 5 / 7)
+            if (de < s_m * Kh && ds > 0.0) {                            // D_edge < L_pix / 2  (Eq. 5 / 7)
                 D.cq = c + off;                                                   // cq != c marks "eligible"
                 if (GEOM == 3) D.a_n = __ldg(absorber + D.cq);
             }
+            // f_c = 1/2 + D_edge / L_pix, L_pix = s_m sqrt(Omega) (R22): geometry too; used only when the
+            // neighbour takes its share (then s_m > 0)
+            D.fc = 0.5 + div_fast(de, s_m * Kl);
         }
         // advance one cell (DEC: s = s_exit; s_a = ((o_a + [d_a > 0]) - 0.5) / d_a)
         s = s_exit;
@@ -291,35 +280,34 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     // P stage: the tests in the oracle's order (box exit, filter, split), then the segment's absorption and
     // its deposit (Eq. 1-2, 5-8).  Returns the ray's outcome.
     auto physics = [&](const SegDesc<IDX> &D) -> int {
-        if (D.a_c == -CUDART_INF) return OUT_EXIT;
-        if (tau >= tau_max) return OUT_KILL_TAU;
-        if (D.split) return OUT_SPLIT;
-        if (D.ds > 0.0) {
-            ++n_seg;
-            const double a_c = fabs(D.a_c);
-            const double dtau = (a_c * sdx) * D.ds;
-            double pm, left;
-            absorb_fraction(dtau, pm, left);
-            const double dN = N * (-pm);
-            if (dN > 0.0) {
-                double fc = 1.0;
-                if (GEOM == 3) {
-                    if (D.a_n > 0.0) {                                            // in the box, absorber > 0, n_H >= n_th
-                        fc = 0.5 + div_fast(D.de, D.s_m * Kl);
-                        atomicAdd(acc + D.cq, (1.0 - fc) * dN);
+        const int outcome = D.a_c == -CUDART_INF ? OUT_EXIT : (tau >= tau_max ? OUT_KILL_TAU : (D.split ? OUT_SPLIT : OUT_NONE));
+        if (outcome == OUT_NONE) {
+            if (D.ds > 0.0) {
+                ++n_seg;
+                const double dtau = (fabs(D.a_c) * sdx) * D.ds;
+                double pm, left;
+                absorb_fraction(dtau, pm, left);
+                const double dN = N * (-pm);
+                if (dN > 0.0) {
+                    double fc = 1.0;
+                    if (GEOM == 3) {
+                        if (D.a_n > 0.0) {                                        // in the box, absorber > 0, n_H >= n_th
+                            fc = D.fc;
+                            atomicAdd(acc + D.cq, (1.0 - fc) * dN);
+                        }
+                    } else if (GEOM == 1 || GEOM == 4) {
+                        if (D.cq != D.c) { fc = D.fc; if (GEOM == 4) fc = fc * fc; }
+                        lost += (1.0 - fc) * dN;
                     }
-                } else if (GEOM == 1 || GEOM == 4) {
-                    if (D.cq != D.c) { fc = 0.5 + div_fast(D.de, D.s_m * Kl); if (GEOM == 4) fc = fc * fc; }
-                    lost += (1.0 - fc) * dN;
+                    atomicAdd(acc + D.c, fc * dN);
                 }
-                atomicAdd(acc + D.c, fc * dN);
+                N = N * left;
+                tau = tau + dtau;
+            } else {
+                ++n_zero;
             }
-            N = N * left;
-            tau = tau + dtau;
-        } else {
-            ++n_zero;
         }
-        return OUT_NONE;
+        return outcome;
     };
 
     // retire rays whose outcome is known (all lanes call it; outcome NONE = nothing to do)
@@ -455,7 +443,10 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 sx1 = (od1 + signed_half(inv1)) * inv1;
                 sx2 = (od2 + signed_half(inv2)) * inv2;
                 has = true;
-                describe(SA);                                                  // first segment: loads in flight
+                // pending segment = a null one (zero length, no deposit): the first pair of the march
+                // describes the real first cell; the null segment's zero-length tally is taken back here
+                SA.a_c = 0.0; SA.a_n = 0.0; SA.ds = 0.0; SA.fc = 1.0; SA.c = c; SA.cq = c; SA.split = false;
+                n_zero -= 1u;
             }
             qhead += take;
             qn -= take;

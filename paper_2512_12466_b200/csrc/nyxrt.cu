@@ -193,6 +193,11 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
     return ((b.off + 255) & ~uint64_t(255));
 }
 
+// default rays per march launch: long batches keep the end-of-launch tail small; the pool is (2 + 5 nlev) B rays
+long long default_batch(const nyxrt_ctx *c) {
+    return c->ncell >= (1ll << 29) ? (1ll << 23) : (c->ncell >= (1ll << 26) ? (1ll << 22) : (1ll << 21));
+}
+
 constexpr size_t MARCH_SMEM = 0;          // the kernel's scratch is static shared memory
 
 template <int GEOM>
@@ -385,7 +390,7 @@ int nyxrt_workspace_bytes(const nyxrt_ctx *cctx, int64_t max_sources, int64_t ba
     if (!ctx || !bytes || max_sources < 0 || batch_rays < 0 || max_sources >= (1ll << 30))
         return fail(ctx, NYXRT_EINVAL, "workspace_bytes: bad argument");
     if (ctx->ws) return fail(ctx, NYXRT_ESTATE, "workspace_bytes: query before set_workspace");
-    const long long B = batch_rays ? batch_rays : (1ll << 21);
+    const long long B = batch_rays ? batch_rays : default_batch(ctx);
     if (B < 32) return fail(ctx, NYXRT_EINVAL, "workspace_bytes: batch_rays must be >= 32");
     *bytes = layout(ctx, nullptr, max_sources, B, host_staging);
     return NYXRT_OK;
@@ -396,7 +401,7 @@ int nyxrt_set_workspace(nyxrt_ctx *ctx, void *d_ws, uint64_t bytes, int64_t max_
     if (!ctx) return NYXRT_EINVAL;
     if (!d_ws || ((uintptr_t)d_ws & 255) || max_sources < 0 || batch_rays < 0 || max_sources >= (1ll << 30))
         return fail(ctx, NYXRT_EINVAL, "set_workspace: bad argument (pointer must be 256-byte aligned)");
-    const long long B = batch_rays ? batch_rays : (1ll << 21);
+    const long long B = batch_rays ? batch_rays : default_batch(ctx);
     if (B < 32) return fail(ctx, NYXRT_EINVAL, "set_workspace: batch_rays must be >= 32");
     ctx->ws = nullptr;
     const uint64_t need = layout(ctx, nullptr, max_sources, B, host_staging);
