@@ -93,19 +93,32 @@ def lognormal_density(n, seed, mean, sigma_ln, device, dtype):
 
 
 def sample_sources(nH, n_src, seed_pos, seed_lum, mean_L, sigma_ln_L):
-    """Cells drawn with probability ~ n_H^2 (inverse CDF on an fp64 cumsum; duplicates allowed, which
-    exercises the dedup pass); luminosities lognormal with the given mean.  Positions are returned in
-    cell units, inside the drawn cell (the library snaps them back)."""
+    """Cells drawn with probability ~ n_H^2 (inverse CDF in fp64; duplicates allowed, which exercises the
+    dedup pass); luminosities lognormal with the given mean.  Positions are returned in cell units, inside
+    the drawn cell (the library snaps them back).
+
+    The inverse CDF is taken in two levels -- x-rows first, then the cell inside the drawn row -- with both
+    running sums made sequentially on the host: a device-wide cumsum on CUDA is not reproducible from run
+    to run (its partial sums are combined in a varying order), and the source list must be."""
     dev = nH.device
     n = nH.shape[0]
-    w = nH.reshape(-1).double()
+    w = nH.reshape(n * n, n).double()
     w = w * w
-    cdf = torch.cumsum(w, 0)
+    rows = w.sum(1).cpu()                                  # per-row reduction: fixed order
+    cdf_r = torch.cumsum(rows, 0)                          # host, sequential
+    total = float(cdf_r[-1])
+    u = torch.rand(n_src, generator=_gen(seed_pos, dev), device=dev, dtype=torch.float64).cpu() * total
+    row = torch.searchsorted(cdf_r, u).clamp_(max=n * n - 1)
+    before = torch.where(row > 0, cdf_r[(row - 1).clamp_(min=0)], torch.zeros_like(u))
+    rem = u - before
+    col = torch.empty(n_src, dtype=torch.int64)
+    step = max(1, (1 << 27) // n)                          # <= 1 GiB of fp64 row copies at a time
+    for a in range(0, n_src, step):
+        r = row[a:a + step]
+        cw = torch.cumsum(w[r.to(dev)].cpu(), 1)           # host, sequential along the row
+        col[a:a + step] = torch.searchsorted(cw, rem[a:a + step, None]).squeeze(1).clamp_(max=n - 1)
     del w
-    total = float(cdf[-1])
-    u = torch.rand(n_src, generator=_gen(seed_pos, dev), device=dev, dtype=torch.float64) * total
-    idx = torch.searchsorted(cdf, u).clamp_(max=cdf.numel() - 1)
-    del cdf
+    idx = (row * n + col).to(dev)
     k = idx // (n * n)
     j = (idx // n) % n
     i = idx % n
