@@ -122,16 +122,15 @@ __device__ __forceinline__ void absorb_fraction(double x, double &pm, double &le
     pm = fma(sc, p, sc - 1.0);
 }
 
-// a / b to a few ulp without the IEEE slow path (not DEC: only scales a deposit); b is a positive normal
-// number.  The hardware seed is good to ~2^-20; one Newton step squares that and the residual correction of
-// the quotient squares it again, so the result is rounding-limited.
+// a / b to ~1e-12 relative without the IEEE slow path (not DEC: only scales a deposit, tolerance 1e-9); b is a
+// positive normal number.  The hardware seed is good to ~2^-20; one Newton step squares that.
 __device__ __forceinline__ double div_fast(double a, double b) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
     const double e = fma(-b, y, 1.0);
     y = fma(y, e, y);
     const double qv = a * y;
-    return fma(fma(-b, qv, a), y, qv);
+    return qv;
 }
 
 // +-1.0 and +-0.5 with the sign of x (x = 1/d: the direction of travel along one axis)
@@ -186,7 +185,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     const long long begin = ls->begin;
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    const double r2s = A.r2_split[level], Kl = A.K[level], Kh = 0.5 * A.K[level];
+    const double r2s = A.r2_split[level], Kl = A.K[level];
+    const double Kh = 0.5 * A.K[level];
     const double tau_max = A.tau_max, sdx = A.sdx;
     const IDX sy = (IDX)A.px, sz = (IDX)A.pxy;
     const double *__restrict__ absorber = A.absorber;
@@ -280,7 +280,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     // P stage: the tests in the oracle's order (box exit, filter, split), then the segment's absorption and
     // its deposit (Eq. 1-2, 5-8).  Returns the ray's outcome.
     auto physics = [&](const SegDesc<IDX> &D) -> int {
-        const int outcome = D.a_c == -CUDART_INF ? OUT_EXIT : (tau >= tau_max ? OUT_KILL_TAU : (D.split ? OUT_SPLIT : OUT_NONE));
+        const bool f_exit = __double2hiint(D.a_c) == (int)0xfff00000;
+        const int outcome = f_exit ? OUT_EXIT : (tau >= tau_max ? OUT_KILL_TAU : (D.split ? OUT_SPLIT : OUT_NONE));
         if (outcome == OUT_NONE) {
             if (D.ds > 0.0) {
                 ++n_seg;
