@@ -95,6 +95,22 @@ def measured_peak():
     return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
 
 
+def max_over_ranks(x, device):
+    """Max of a scalar over all ranks (the contract's timing rule); identity when not distributed."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank, ms_max, world):
+    """Replicas only: every rank processes `units_per_rank`; the job's rate is all
+    ranks' units over the slowest rank's time."""
+    return world * units_per_rank / (ms_max * 1e-3)
+
+
 def make_workload(args, device):
     from paper_2512_12466_b200 import synth
     cfg = synth.make(args.config, device=device)
@@ -218,11 +234,8 @@ def main():
     barrier()
     ms = e0.elapsed_time(e1)
     clk = clocks.stop() if rank == 0 else None
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * seg / (ms * 1e-3)
+    ms = max_over_ranks(ms, "cuda")
+    value = whole_job_rate(seg, ms, world)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
@@ -240,11 +253,8 @@ def main():
             seg_e += tr.step_host(h_nH, h_xHI, pos, L, h_g, h_h).segments
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
-        e2e = dict(value=world * seg_e / dt, unit="segments/s", steps=ke, ms_per_step=1e3 * dt / ke,
+        dt = max_over_ranks(dt, "cuda")
+        e2e = dict(value=whole_job_rate(seg_e, dt * 1e3, world), unit="segments/s", steps=ke, ms_per_step=1e3 * dt / ke,
                    h2d_bytes_per_step=int(2 * h_nH.numel() * h_nH.element_size() + pos.nbytes + L.nbytes),
                    d2h_bytes_per_step=int(2 * h_g.numel() * 8),
                    checksum_gamma_sum=float(h_g.sum()))

@@ -73,7 +73,6 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
     ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 2 : (pick < 4 ? 4 : (pick < 6 ? 8 : 16)));
-    ls->refill_min = ls->tune_refill_min > 0 ? ls->tune_refill_min : 6;
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
@@ -122,15 +121,18 @@ __device__ __forceinline__ void absorb_fraction(double x, double &pm, double &le
     pm = fma(sc, p, sc - 1.0);
 }
 
-// a / b to ~1e-12 relative without the IEEE slow path (not DEC: only scales a deposit, tolerance 1e-9); b is a
-// positive normal number.  The hardware seed is good to ~2^-20; one Newton step squares that.
+// a / b to a few ulp without the IEEE slow path (not DEC: only scales a deposit); b is a positive normal
+// number.  The hardware seed is good to ~2^-20; one Newton step squares that and the residual correction of
+// the quotient squares it again, so the result is rounding-limited.  (The correction is needed: the
+// neighbour's share is 1 - f_c = 1/2 - a/b, which cancels when D_edge is close to L_pix/2, and a cell may
+// receive nothing but such shares.)
 __device__ __forceinline__ double div_fast(double a, double b) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(b));
     const double e = fma(-b, y, 1.0);
     y = fma(y, e, y);
     const double qv = a * y;
-    return qv;
+    return fma(fma(-b, qv, a), y, qv);
 }
 
 // +-1.0 and +-0.5 with the sign of x (x = 1/d: the direction of travel along one axis)

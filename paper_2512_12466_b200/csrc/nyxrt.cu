@@ -45,7 +45,7 @@ struct nyxrt_ctx {
     nyxrt_params p;
     char err[512];
     int sm_count, march_blocks, nlev;
-    int tune_seg_round, tune_refill_min;   // NYXRT_SEG_ROUND / NYXRT_REFILL_MIN (tuning knobs, 0 = scheduler's choice)
+    int tune_seg_round;                    // NYXRT_SEG_ROUND (tuning knob, 0 = scheduler's choice)
     long long ncell;
     // workspace
     void *ws;
@@ -366,7 +366,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     ctx->sm_count = prop.multiProcessorCount;
     ctx->march_blocks = ctx->sm_count * (occ > 0 ? occ : 1);
     if (const char *v = getenv("NYXRT_SEG_ROUND")) ctx->tune_seg_round = atoi(v);
-    if (const char *v = getenv("NYXRT_REFILL_MIN")) ctx->tune_refill_min = atoi(v);
     *out = ctx;
     return NYXRT_OK;
 }
@@ -501,7 +500,6 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     ctx->h_ls->n_cat = ctx->n_cat;
     ctx->h_ls->batch_rays = ctx->batch_rays;
     ctx->h_ls->tune_seg_round = ctx->tune_seg_round;
-    ctx->h_ls->tune_refill_min = ctx->tune_refill_min;
     CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
     MarchArgs a;
     memset(&a, 0, sizeof a);

@@ -31,9 +31,8 @@ struct LoopState {
     int level;
     int done;
     int overflow;
-    int seg_round;                       // segments marched between two refills of idle lanes
-    int refill_min;                      // idle lanes of a warp that trigger a refill
-    int tune_seg_round, tune_refill_min; // > 0: override the scheduler's choice (tuning knobs)
+    int seg_round;                       // cells marched per round, between two retire / pop passes
+    int tune_seg_round;                  // > 0: overrides the scheduler's choice (tuning knob)
     unsigned long long iterations, peak_pool;
     unsigned long long fetch;            // next unclaimed ray of the current batch (chunks of FETCH_CHUNK)
 };

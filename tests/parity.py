@@ -92,3 +92,28 @@ def compare(res_gpu, res_or, cfg, params=None):
         assert abs(a - b) <= 1e-11 * max(abs(b), 1e-300) + 1e-11 * so.photons_emitted * (f != "photons_emitted"), (f, a, b)
     rel = err / np.maximum(np.abs(go), 1e-300)
     return float(rel[go != 0].max()) if (go != 0).any() else 0.0
+
+
+def compare_slabs(gam_gpu, heat_gpu, go, ho, cfg, params=None, slab=32):
+    """The per-cell rule of `compare` for a grid too large to hold several host copies of: the GPU result
+    stays on the device, the oracle's arrays (numpy) are brought over z-slab by z-slab."""
+    p = dict(cfg["params"])
+    p.update(params or {})
+    worst = 0.0
+    nz = gam_gpu.shape[0]
+    for z0 in range(0, nz, slab):
+        z1 = min(nz, z0 + slab)
+        o = torch.from_numpy(go[z0:z1]).to(gam_gpu.device)
+        g = gam_gpu[z0:z1]
+        err = (g - o).abs()
+        assert not bool((err > RTOL * o.abs() + ATOL).any()), ("Gamma", z0)
+        assert bool(((g == 0) == (o == 0)).all()), ("Gamma zero pattern", z0)
+        nz_mask = o != 0
+        if bool(nz_mask.any()):
+            worst = max(worst, float((err[nz_mask] / o[nz_mask].abs()).max()))
+        if heat_gpu is not None and ho is not None:
+            h = torch.from_numpy(ho[z0:z1]).to(gam_gpu.device)
+            nHI = cfg["nH"][z0:z1].double() * cfg["xHI"][z0:z1].double()
+            floor = ATOL * p["e_excess_erg"] * nHI
+            assert not bool(((heat_gpu[z0:z1] - h).abs() > RTOL * h.abs() + floor).any()), ("heat", z0)
+    return worst

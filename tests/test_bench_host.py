@@ -1,0 +1,48 @@
+"""Host logic of bench.py's N > 1 path ("replicas only": no data-path collective; the only exchange is the
+max-over-ranks of the timing), run as two gloo ranks on the CPU; and the --impl reference rule that only
+rank 0 works."""
+import os
+import subprocess
+import sys
+
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    sys.path.insert(0, ROOT)
+    import bench
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms = bench.max_over_ranks(100.0 + 50.0 * rank, "cpu")        # rank 1 is the slow one
+    out[rank] = (ms, bench.whole_job_rate(1000, ms, world))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_replicas_rate_is_all_units_over_slowest_rank():
+    world = 2
+    with mp.Manager() as m:
+        out = m.dict()
+        mp.spawn(_worker, args=(world, 29533, out), nprocs=world, join=True)
+        res = dict(out)
+    assert res[0] == res[1]
+    ms, rate = res[0]
+    assert ms == 150.0 and abs(rate - 2 * 1000 / 0.150) < 1e-9
+
+
+def test_single_process_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.max_over_ranks(12.5, "cpu") == 12.5
+    assert bench.whole_job_rate(10, 1000.0, 1) == 10.0
+
+
+def test_reference_arm_other_ranks_exit_quietly():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
+                       env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and r.stdout.strip() == ""
