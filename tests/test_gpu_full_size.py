@@ -100,3 +100,24 @@ def test_config5_full_step_properties(cfg5):
     assert all(np.array_equal(a, b) for a, b in zip(cat, cat2))
     assert bool(((gam2 - gam).abs() <= 1e-11 * gam).all())
     assert abs(st2.photons_absorbed - st.photons_absorbed) <= BUDGET_RTOL * st.photons_emitted
+
+
+@pytest.mark.parametrize("config_id,n_sample", [(3, 40), (4, 3)])
+def test_configs_3_4_full_grid_sampled_sources(O, config_id, n_sample):
+    """Configs 3 (256^3, merging off) and 4 (512^3, merging on), fp64 fields: the full grid, a sample of the
+    source list the oracle finishes in seconds, element by element."""
+    cfg = synth.make(config_id, device="cuda")
+    pos, L = cfg["src_pos"].numpy()[:n_sample], cfg["src_L"].numpy()[:n_sample]
+    gam, heat, sg, cg = _trace(cfg, pos, L)
+    sub = dict(cfg)
+    sub["src_pos"], sub["src_L"] = cfg["src_pos"][:n_sample], cfg["src_L"][:n_sample]
+    go, ho, so, co = run_oracle(O, sub)
+    assert np.array_equal(cg[0], co[0]) and np.array_equal(cg[1], co[1]) and np.array_equal(cg[2], co[2])
+    for name in COUNTERS:
+        assert list(getattr(sg, name)) == list(getattr(so, name)), name
+    assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    worst = compare_slabs(gam, heat, go, ho, cfg)
+    assert_budget(sg, "gpu")
+    assert_budget(so, "oracle")
+    print("config %d full grid, %d sources: %d segments, worst relative Gamma error %.2e"
+          % (config_id, n_sample, sg.segments, worst))
