@@ -121,3 +121,33 @@ def test_configs_3_4_full_grid_sampled_sources(O, config_id, n_sample):
     assert_budget(so, "oracle")
     print("config %d full grid, %d sources: %d segments, worst relative Gamma error %.2e"
           % (config_id, n_sample, sg.segments, worst))
+
+
+def test_64bit_cell_index_path(O):
+    """Maximum size: a padded grid of more than 2^31 cells switches the march to 64-bit cell indices
+    (march_kernel<GEOM, long long>).  Non-cubic 1026 x 1022 x 2046 fp32 grid, moderately thick medium so that
+    the oracle finishes in seconds, sources at both ends of the index range (the last one in the far corner,
+    linear index > 2^31) and next to three faces."""
+    if torch.cuda.mem_get_info()[1] < 150e9:
+        pytest.skip("needs the B200's memory")
+    nz, ny, nx = 1026, 1022, 2046
+    assert (nz + 2) * (ny + 2) * (nx + 2) >= 2 ** 31
+    g = torch.Generator(device="cuda").manual_seed(64)
+    nH = (torch.rand((nz, ny, nx), generator=g, device="cuda", dtype=torch.float32) + 0.5) * 1e-3
+    xHI = torch.rand((nz, ny, nx), generator=g, device="cuda", dtype=torch.float32) * 0.8 + 0.2
+    cfg = dict(name="idx64", n=None, shape=(nz, ny, nx), dx_cm=1.3e20, nH=nH, xHI=xHI,
+               src_pos=torch.tensor([[3.5, 2.5, 1.5], [2042.2, 1018.7, 1022.1], [1000.5, 500.5, 1024.9],
+                                     [2045.9, 1021.9, 1025.9]], dtype=torch.float64),
+               src_L=torch.tensor([1e50, 3e50, 2e49, 5e50], dtype=torch.float64),
+               params=synth.default_params(n_th=6e-4, e_excess_erg=1e-11))
+    gam, heat, sg, cg = _trace(cfg, cfg["src_pos"].numpy(), cfg["src_L"].numpy(), batch_rays=2 ** 20)
+    go, ho, so, co = run_oracle(O, cfg)
+    assert np.array_equal(cg[0], co[0]) and np.array_equal(cg[1], co[1])
+    for name in COUNTERS:
+        assert list(getattr(sg, name)) == list(getattr(so, name)), name
+    assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    assert sum(sg.exited) > 0 and sum(sg.killed_tau) > 0 and sg.segments > 10 ** 6
+    worst = compare_slabs(gam, heat, go, ho, cfg)
+    assert float(gam[-1, -1, -1]) > 0.0                       # the far corner cell (largest index) was lit
+    assert_budget(sg, "gpu")
+    print("64-bit index path: %d segments, worst relative Gamma error %.2e" % (sg.segments, worst))
