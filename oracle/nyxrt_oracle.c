@@ -52,6 +52,8 @@ typedef struct {
     double  dx_cm;            /* cubic cell width */
     double  box_lo[3];        /* low corner of cell (0,0,0), in position units */
     double  pos_unit_cm;      /* cm per position unit */
+    int32_t periodic;         /* 0: rays leaving the box are removed (R20); 1: periodic box */
+    int32_t pad_;
 } orc_grid;
 
 typedef struct {
@@ -246,6 +248,19 @@ static int64_t lin(const orc_grid *g, int64_t i, int64_t j, int64_t k) {
     return (k * g->ny + j) * (int64_t)g->nx + i;
 }
 
+/* periodic box ("rays wrap around the box"): index into [0, n) */
+static int64_t wrap(int64_t i, int64_t n) {
+    i %= n;
+    return i < 0 ? i + n : i;
+}
+
+/* minimum-image difference of two cell coordinates ("minimum-image convention"): the
+   representative of a - b (mod n) in [-n/2, n/2); for even n the tie n/2 maps to -n/2 (reading R31) */
+static int64_t minimg(int64_t d, int64_t n) {
+    d = wrap(d, n);
+    return (2 * d >= n) ? d - n : d;
+}
+
 int orc_bubble_radius(const orc_grid *g, const orc_params *p, const void *xHI, int64_t n,
                       const int32_t *cell, double *r_out) {
     if (p->samp_level < 0 || p->samp_level > 8 || !(p->delta_r > 0.0)) return ORC_EINVAL;
@@ -264,7 +279,8 @@ int orc_bubble_radius(const orc_grid *g, const orc_params *p, const void *xHI, i
                 int64_t i = c[0] + (int64_t)floor(fma(r, dir[3 * q + 0], 0.5));
                 int64_t j = c[1] + (int64_t)floor(fma(r, dir[3 * q + 1], 0.5));
                 int64_t k = c[2] + (int64_t)floor(fma(r, dir[3 * q + 2], 0.5));
-                if (!in_box(g, i, j, k)) continue;                            /* "checked" samples */
+                if (g->periodic) { i = wrap(i, g->nx); j = wrap(j, g->ny); k = wrap(k, g->nz); }  /* PAPER.md:351 */
+                else if (!in_box(g, i, j, k)) continue;                       /* "checked" samples */
                 ++ntot;
                 double x = 1.0 - fld(xHI, g->field_dtype, lin(g, i, j, k));
                 if (x >= p->x_th) ++nion;
@@ -313,6 +329,7 @@ int orc_merge(const orc_grid *g, const orc_params *p, int64_t n, const int32_t *
             if (!(r[b] > 0.0)) continue;
             int64_t dx = (int64_t)cell[3 * a] - cell[3 * b], dy = (int64_t)cell[3 * a + 1] - cell[3 * b + 1],
                     dz = (int64_t)cell[3 * a + 2] - cell[3 * b + 2];
+            if (g->periodic) { dx = minimg(dx, g->nx); dy = minimg(dy, g->ny); dz = minimg(dz, g->nz); }  /* PAPER.md:321 */
             int64_t d2 = dx * dx + dy * dy + dz * dz;
             double rs = p->f_ov * (r[a] + r[b]);                              /* PAPER.md:327 */
             if ((double)d2 <= rs * rs + p->eps) {                             /* PAPER.md:331 */
@@ -336,19 +353,29 @@ int orc_merge(const orc_grid *g, const orc_params *p, int64_t n, const int32_t *
             M.c[0] = cell[3 * a]; M.c[1] = cell[3 * a + 1]; M.c[2] = cell[3 * a + 2];
             M.L = L[a]; M.r = r[a];
         } else {
+            const int64_t nn[3] = { g->nx, g->ny, g->nz };
             double F = 0.0, R = 0.0, num[3] = { 0.0, 0.0, 0.0 };
             for (int64_t b = a; b < n; ++b) {                                 /* member order */
                 if (uf_find(par, b) != ra) continue;
                 F = F + L[b];
                 if (r[b] > R) R = r[b];
-                for (int ax = 0; ax < 3; ++ax) num[ax] = num[ax] + L[b] * (double)cell[3 * b + ax];
+                for (int ax = 0; ax < 3; ++ax) {
+                    /* periodic: x'_m = x_ref + minimg(x_m - x_ref), reference = first member */
+                    int64_t x = cell[3 * b + ax];
+                    if (g->periodic) x = cell[3 * a + ax] + minimg(x - cell[3 * a + ax], nn[ax]);
+                    num[ax] = num[ax] + L[b] * (double)x;
+                }
             }
             int64_t rc[3];
-            for (int ax = 0; ax < 3; ++ax) rc[ax] = (int64_t)floor(num[ax] / F + 0.5);  /* R9 */
+            for (int ax = 0; ax < 3; ++ax) {
+                rc[ax] = (int64_t)floor(num[ax] / F + 0.5);                   /* R9 */
+                if (g->periodic) rc[ax] = wrap(rc[ax], nn[ax]);               /* "wrapped back into the box" */
+            }
             int64_t best = -1, bestd = 0;
             for (int64_t b = a; b < n; ++b) {                                 /* snap */
                 if (uf_find(par, b) != ra) continue;
                 int64_t dx = cell[3 * b] - rc[0], dy = cell[3 * b + 1] - rc[1], dz = cell[3 * b + 2] - rc[2];
+                if (g->periodic) { dx = minimg(dx, g->nx); dy = minimg(dy, g->ny); dz = minimg(dz, g->nz); }
                 int64_t d2 = dx * dx + dy * dy + dz * dz;
                 if (best < 0 || d2 < bestd) { best = b; bestd = d2; }         /* first minimum, R10 */
             }
@@ -381,6 +408,7 @@ typedef struct {
     int64_t log_cap, log_n;
     double r2_split[ORC_MAXLEV], K[ORC_MAXLEV];
     double sdx, V;
+    double s_max;             /* periodic: sqrt(nx^2 + ny^2 + nz^2) cells = sqrt(3) L_box for a cube */
     long double absorbed, escaped, residual, lost;
     int32_t src_cell[3];
     int32_t src_id;
@@ -408,7 +436,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
             sx[a] = ((double)(o[a] + (d[a] > 0.0 ? 1 : 0)) - 0.5) * inv[a];
         }
     }
-    if (!in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
+    if (!g->periodic && !in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
         st->exited[level]++;
         T->escaped += (long double)(L_ray * exp(-tau));
         return;
@@ -424,6 +452,13 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
         if (level >= p->level_max) {
             st->killed_lmax[level]++;
             T->residual += (long double)(L_ray * exp(-tau));
+            return;
+        }
+        /* 2b. periodic box: the ray ends once its travel distance is no longer below sqrt(3) L_box
+           (RAY_FLTR); counted with the rays that left the system (reading R30) */
+        if (g->periodic && !(s < T->s_max)) {
+            st->exited[level]++;
+            T->escaped += (long double)(L_ray * exp(-tau));
             return;
         }
         /* 3. split, Eq. 4: Omega_c/Omega(l) < N_min  <=>  s^2 > 3 4^l/(pi N_min) */
@@ -442,6 +477,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
         if (ds > 0.0) {
             st->segments++;
             int64_t ci = T->src_cell[0] + o[0], cj = T->src_cell[1] + o[1], ck = T->src_cell[2] + o[2];
+            if (g->periodic) { ci = wrap(ci, g->nx); cj = wrap(cj, g->ny); ck = wrap(ck, g->nz); }  /* PAPER.md:132 */
             int64_t c = lin(g, ci, cj, ck);
             double nH_c = fld(T->nH, g->field_dtype, c);
             double a_c = nH_c * fld(T->xHI, g->field_dtype, c);        /* absorber density, PAPER.md:229 (R1) */
@@ -472,6 +508,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
                         else {                                         /* 2: Eq. 5-6; 3: Eq. 7-8 */
                             int64_t nb[3] = { ci, cj, ck };
                             nb[face >> 1] += (face & 1) ? 1 : -1;
+                            if (g->periodic) { nb[0] = wrap(nb[0], g->nx); nb[1] = wrap(nb[1], g->ny); nb[2] = wrap(nb[2], g->nz); }
                             if (in_box(g, nb[0], nb[1], nb[2])) {      /* R23 */
                                 int64_t q = lin(g, nb[0], nb[1], nb[2]);
                                 double nH_n = fld(T->nH, g->field_dtype, q);
@@ -522,7 +559,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
         s = s_exit;
         o[ax] += (d[ax] > 0.0) ? 1 : -1;
         sx[ax] = ((double)(o[ax] + (d[ax] > 0.0 ? 1 : 0)) - 0.5) * inv[ax];
-        if (!in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
+        if (!g->periodic && !in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
             st->exited[level]++;                                        /* R20 */
             T->escaped += (long double)(L_ray * exp(-tau));
             return;
@@ -551,6 +588,7 @@ int orc_trace(const orc_grid *g, const orc_params *p, const void *nH, const void
     }
     T.sdx = p->sigma_cm2 * g->dx_cm;
     T.V = g->dx_cm * g->dx_cm * g->dx_cm;                              /* V_box = h^3 */
+    T.s_max = sqrt((double)((int64_t)g->nx * g->nx + (int64_t)g->ny * g->ny + (int64_t)g->nz * g->nz));
     long double emitted = 0.0L;
     for (int64_t a = 0; a < n_cat; ++a) {
         T.src_cell[0] = cell[3 * a]; T.src_cell[1] = cell[3 * a + 1]; T.src_cell[2] = cell[3 * a + 2];

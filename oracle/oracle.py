@@ -28,7 +28,8 @@ def build(force=False):
 
 class Grid(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("field_dtype", C.c_int32),
-                ("dx_cm", C.c_double), ("box_lo", C.c_double * 3), ("pos_unit_cm", C.c_double)]
+                ("dx_cm", C.c_double), ("box_lo", C.c_double * 3), ("pos_unit_cm", C.c_double),
+                ("periodic", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Params(C.Structure):
@@ -75,8 +76,9 @@ def lib():
     return _lib
 
 
-def make_grid(shape_zyx, dx_cm, field_dtype=np.float64, box_lo=(0.0, 0.0, 0.0), pos_unit_cm=None):
+def make_grid(shape_zyx, dx_cm, field_dtype=np.float64, box_lo=(0.0, 0.0, 0.0), pos_unit_cm=None, periodic=0):
     g = Grid()
+    g.periodic = int(periodic)
     g.nz, g.ny, g.nx = [int(v) for v in shape_zyx]
     g.field_dtype = 1 if np.dtype(field_dtype) == np.float32 else 0
     g.dx_cm = float(dx_cm)
