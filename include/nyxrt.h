@@ -45,7 +45,11 @@ typedef struct {
     double  dx_cm;             /* cell width h in cm; V_box = h^3 (PAPER.md:205 footnote 2)         */
     double  box_lo[3];         /* position of the low corner of cell (0,0,0), in position units     */
     double  pos_unit_cm;       /* cm per position unit of nyxrt_set_sources (dx_cm => cell units)    */
-    int32_t periodic;          /* must be 0: rays die on leaving the box (BASELINE.json; R20)       */
+    int32_t periodic;          /* 0: rays die on leaving the box (BASELINE.json configs; R20);
+                                  1: periodic box: cells wrap, a ray ends once its travel
+                                  distance reaches sqrt(nx^2+ny^2+nz^2) cells (= sqrt(3) L_box, PAPER.md:174;
+                                  counted in exited[] / photons_escaped, R30), minimum-image merge and wrapped
+                                  shell samples (tie rule R31)                */
     int32_t device;            /* CUDA device ordinal                                               */
 } nyxrt_grid;
 
@@ -96,7 +100,7 @@ typedef struct {
 } nyxrt_stats;
 
 /* Create a context for one grid.  Copies *grid and *params.  Allocates only small bookkeeping
- * (host + a few KB device).  Errors: EINVAL (bad sizes / parameters, periodic != 0), ECUDA. */
+ * (host + a few KB device).  Errors: EINVAL (bad sizes / parameters, periodic not 0 or 1), ECUDA. */
 int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx **out);
 
 /* Size of the caller-provided device workspace.

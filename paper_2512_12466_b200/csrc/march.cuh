@@ -158,7 +158,8 @@ struct SegDesc {
     double a_c, a_n;      // absorber of the cell (sign = Eq. 7-8 flag, -inf = outside the box) and of the neighbour
     double ds, fc;        // length; f_c = 1/2 + D_edge / L_pix of Eq. 5 / 7
     IDX c, cq;            // cell and neighbour across the nearest face (cq == c: no neighbour deposit)
-    bool split;           // the cell's entry distance meets Eq. 4: the ray splits here instead of marching
+    int split;            // 1: the cell's entry distance meets Eq. 4: the ray splits here instead of marching;
+                          // 2 (periodic box): the entry distance is no longer below sqrt(3) L_box: the ray ends
 };
 
 // Rays of the current chunk that passed their birth tests, initialised at full warp width and parked until
@@ -171,10 +172,19 @@ struct RayQueue {
     double d0[MARCH_WARPS][32], d1[MARCH_WARPS][32], d2[MARCH_WARPS][32];           // HEALPix direction
     double inv0[MARCH_WARPS][32], inv1[MARCH_WARPS][32], inv2[MARCH_WARPS][32];     // 1/d (-inf where d = 0)
     IDX c[MARCH_WARPS][32];                                                          // start cell
+    unsigned long long cnt[MARCH_WARPS][32];                                         // periodic box: steps to each face
 };
 
+// Periodic box: the ray's cell index stays inside the box.  cnt packs, 21 bits per
+// axis, the number of steps the ray can still take along that axis before it crosses the box face;
+// the step that crosses lands on the opposite side instead (c moves by (1 - n) strides).
+constexpr int WRAP_BITS = 21;
+constexpr unsigned long long WRAP_MASK = (1ull << WRAP_BITS) - 1ull;
+
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
-template <int GEOM, typename IDX>
+// PER: periodic box: cells wrap, rays end at s >= sqrt(3) L_box, the halo holds the wrapped
+// images of the opposite faces (neighbour reads) and deposits into it are folded back by finalise.
+template <int GEOM, typename IDX, bool PER>
 __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(const __grid_constant__ MarchArgs A) {
     __shared__ ThreadScratch T;
     __shared__ RayQueue<IDX> Q;
@@ -190,6 +200,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     const double r2s = A.r2_split[level], Kl = A.K[level];
     const double Kh = 0.5 * A.K[level];
     const double tau_max = A.tau_max, sdx = A.sdx;
+    const double s_max = A.s_max;
     const IDX sy = (IDX)A.px, sz = (IDX)A.pxy;
     const double *__restrict__ absorber = A.absorber;
     double *__restrict__ acc = A.acc;
@@ -211,8 +222,9 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     double s = 0.0, tau = 0.0, N = 0.0;
     double d0 = 0, d1 = 0, d2 = 0, inv0 = 0, inv1 = 0, inv2 = 0, od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
     IDX c = 0, cst0 = 0, cst1 = 0, cst2 = 0;       // cell (padded linear index) and its signed step per axis
+    unsigned long long cnt = 0;                    // periodic box: steps left to the faces (3 x 21 bits)
     SegDesc<IDX> SA, SB;
-    SA.split = SB.split = false;
+    SA.split = SB.split = 0;
 
     // G stage: describe the cell the DDA stands in (everything here is geometry: no loaded value is needed),
     // issue its absorber loads, and advance the DDA to the next cell.  A cell that meets the split criterion
@@ -221,11 +233,12 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     auto describe = [&](SegDesc<IDX> &D) {
         D.c = c;
         D.a_c = __ldg(absorber + c);
-        const bool split = s * s > r2s;
-        D.split = split;
+        int flag = s * s > r2s ? 1 : 0;
+        if (PER && !(s < s_max)) flag = 2;                                        // RAY_FLTR, PAPER.md:174 (before split)
+        D.split = flag;
         D.cq = c;
         D.a_n = 0.0;
-        if (split) return;                                                        // rare: once per ray at most
+        if (flag) return;                                                         // rare: once per ray at most
         double s_exit = sx0; int ax = 0;
         if (sx1 < s_exit) { s_exit = sx1; ax = 1; }
         if (sx2 < s_exit) { s_exit = sx2; ax = 2; }                               // first minimum, order x, y, z
@@ -276,14 +289,32 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         if (ax == 0) { od0 += signed_one(inv0); sx0 = (od0 + signed_half(inv0)) * inv0; }
         if (ax == 1) { od1 += signed_one(inv1); sx1 = (od1 + signed_half(inv1)) * inv1; }
         if (ax == 2) { od2 += signed_one(inv2); sx2 = (od2 + signed_half(inv2)) * inv2; }
-        c += ax == 0 ? cst0 : (ax == 1 ? cst1 : cst2);
+        const IDX stp = ax == 0 ? cst0 : (ax == 1 ? cst1 : cst2);
+        if (PER) {
+            const int sh = WRAP_BITS * ax;
+            const int n_ax = ax == 0 ? A.nx : (ax == 1 ? A.ny : A.nz);
+            if (((cnt >> sh) & WRAP_MASK) == 0ull) {                              // crosses the face: wrap around
+                c += stp - stp * (IDX)n_ax;
+                cnt += (unsigned long long)(n_ax - 1) << sh;
+            } else {
+                c += stp;
+                cnt -= 1ull << sh;
+            }
+        } else {
+            c += stp;
+        }
     };
 
     // P stage: the tests in the oracle's order (box exit, filter, split), then the segment's absorption and
     // its deposit (Eq. 1-2, 5-8).  Returns the ray's outcome.
     auto physics = [&](const SegDesc<IDX> &D) -> int {
-        const bool f_exit = __double2hiint(D.a_c) == (int)0xfff00000;
-        const int outcome = f_exit ? OUT_EXIT : (tau >= tau_max ? OUT_KILL_TAU : (D.split ? OUT_SPLIT : OUT_NONE));
+        int outcome;
+        if (PER) {
+            outcome = tau >= tau_max ? OUT_KILL_TAU : (D.split == 2 ? OUT_EXIT : (D.split ? OUT_SPLIT : OUT_NONE));
+        } else {
+            const bool f_exit = __double2hiint(D.a_c) == (int)0xfff00000;
+            outcome = f_exit ? OUT_EXIT : (tau >= tau_max ? OUT_KILL_TAU : (D.split ? OUT_SPLIT : OUT_NONE));
+        }
         if (outcome == OUT_NONE) {
             if (D.ds > 0.0) {
                 ++n_seg;
@@ -382,6 +413,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             if (lane == 0) n_hole += __popc(m_hole);
             double ts = 0.0, ttau = 0.0, tN = 0.0, e0 = 0.0, e1 = 0.0, e2 = 0.0, i0 = 0.0, i1 = 0.0, i2 = 0.0;
             IDX tc = 0;
+            unsigned long long tcnt = 0;
             bool park = false;
             if (real) {
                 ts = A.pool.s[r];
@@ -397,10 +429,19 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 i0 = (e0 == 0.0) ? -CUDART_INF : 1.0 / e0;                     // with od + (-0.5): s_x = +inf
                 i1 = (e1 == 0.0) ? -CUDART_INF : 1.0 / e1;
                 i2 = (e2 == 0.0) ? -CUDART_INF : 1.0 / e2;
-                const long long ci = sc.x + (long long)o0, cj = sc.y + (long long)o1, ck = sc.z + (long long)o2;
-                if (ci < 0 || ci >= A.nx || cj < 0 || cj >= A.ny || ck < 0 || ck >= A.nz) outcome = OUT_EXIT;
+                long long ci = sc.x + (long long)o0, cj = sc.y + (long long)o1, ck = sc.z + (long long)o2;
+                if (PER) {
+                    ci %= A.nx; if (ci < 0) ci += A.nx;
+                    cj %= A.ny; if (cj < 0) cj += A.ny;
+                    ck %= A.nz; if (ck < 0) ck += A.nz;
+                    tcnt = (unsigned long long)(e0 > 0.0 ? A.nx - 1 - ci : ci) |
+                           ((unsigned long long)(e1 > 0.0 ? A.ny - 1 - cj : cj) << WRAP_BITS) |
+                           ((unsigned long long)(e2 > 0.0 ? A.nz - 1 - ck : ck) << (2 * WRAP_BITS));
+                }
+                if (!PER && (ci < 0 || ci >= A.nx || cj < 0 || cj >= A.ny || ck < 0 || ck >= A.nz)) outcome = OUT_EXIT;
                 else if (ttau >= tau_max) outcome = OUT_KILL_TAU;
                 else if (level >= A.level_max) outcome = OUT_KILL_LMAX;
+                else if (PER && !(ts < s_max)) outcome = OUT_EXIT;
                 else if (ts * ts > r2s) outcome = OUT_SPLIT;
                 else {
                     tc = (IDX)(((ck + 1) * A.pxy) + (cj + 1) * A.px + (ci + 1));
@@ -415,6 +456,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 Q.d0[wid][e] = e0; Q.d1[wid][e] = e1; Q.d2[wid][e] = e2;
                 Q.inv0[wid][e] = i0; Q.inv1[wid][e] = i1; Q.inv2[wid][e] = i2;
                 Q.c[wid][e] = tc;
+                if (PER) Q.cnt[wid][e] = tcnt;
             }
             qhead = 0;
             qn = __popc(m_park);
@@ -435,6 +477,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 d0 = Q.d0[wid][e]; d1 = Q.d1[wid][e]; d2 = Q.d2[wid][e];
                 inv0 = Q.inv0[wid][e]; inv1 = Q.inv1[wid][e]; inv2 = Q.inv2[wid][e];
                 c = Q.c[wid][e];
+                if (PER) cnt = Q.cnt[wid][e];
                 double q;
                 q = fma(s, d0, 0.5); od0 = floor(q); if (q == od0 && d0 < 0.0) od0 -= 1.0;
                 q = fma(s, d1, 0.5); od1 = floor(q); if (q == od1 && d1 < 0.0) od1 -= 1.0;
@@ -448,7 +491,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 has = true;
                 // pending segment = a null one (zero length, no deposit): the first pair of the march
                 // describes the real first cell; the null segment's zero-length tally is taken back here
-                SA.a_c = 0.0; SA.a_n = 0.0; SA.ds = 0.0; SA.fc = 1.0; SA.c = c; SA.cq = c; SA.split = false;
+                SA.a_c = 0.0; SA.a_n = 0.0; SA.ds = 0.0; SA.fc = 1.0; SA.c = c; SA.cq = c; SA.split = 0;
                 n_zero -= 1u;
             }
             qhead += take;
@@ -512,21 +555,25 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
 // for automerge.
 template <typename T>
 __global__ void prep_fields_kernel(const T *__restrict__ nH, const T *__restrict__ xHI, double *__restrict__ a,
-                                   int nx, int ny, int nz, double n_th, int use_flag,
+                                   int nx, int ny, int nz, double n_th, int use_flag, int periodic,
                                    double *__restrict__ partial) {
     __shared__ double sh[256];
     double acc = 0.0;
     const long long px = nx + 2, py = ny + 2, pz = nz + 2, ptot = px * py * pz;
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < ptot;
          q += (long long)gridDim.x * blockDim.x) {
-        const long long i = q % px - 1, j = (q / px) % py - 1, k = q / (px * py) - 1;
+        long long i = q % px - 1, j = (q / px) % py - 1, k = q / (px * py) - 1;
         double v = -CUDART_INF;
-        if (i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz) {
+        const bool inside = i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz;
+        if (periodic) {                            // halo = image of the opposite side
+            i = (i + nx) % nx; j = (j + ny) % ny; k = (k + nz) % nz;
+        }
+        if (inside || periodic) {
             const long long t = (k * ny + j) * nx + i;
             const double n = (double)nH[t], x = (double)xHI[t];
             v = n * x;
             if (use_flag && !(n >= n_th)) v = -v;
-            acc += 1.0 - x;
+            if (inside) acc += 1.0 - x;
         }
         a[q] = v;
     }
@@ -559,7 +606,7 @@ __global__ void sum_partials_kernel(const double *partial, int n, double *out) {
 // absorber, writes the caller's dense [nz][ny][nx] outputs.
 __global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__ heat, const double *__restrict__ acc,
                                 const double *__restrict__ absorber, int nx, int ny, int nz, double V,
-                                double e_excess, double *__restrict__ partial) {
+                                double e_excess, int periodic, double *__restrict__ partial) {
     __shared__ double sh[256];
     double sum = 0.0;
     const long long ncell = (long long)nx * ny * nz, px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2);
@@ -567,7 +614,17 @@ __global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__
          t += (long long)gridDim.x * blockDim.x) {
         const long long i = t % nx, j = (t / nx) % ny, k = t / ((long long)nx * ny);
         const long long q = (k + 1) * pxy + (j + 1) * px + (i + 1);
-        const double ph = acc[q];
+        double ph = acc[q];
+        if (periodic) {
+            // neighbour shares deposited across a box face went to the halo image of the cell on the
+            // opposite side: fold them back (only face halos can hold any: a neighbour differs in one axis)
+            if (i == 0) ph += acc[q + nx];
+            if (i == nx - 1) ph += acc[q - nx];
+            if (j == 0) ph += acc[q + ny * px];
+            if (j == ny - 1) ph += acc[q - ny * px];
+            if (k == 0) ph += acc[q + nz * pxy];
+            if (k == nz - 1) ph += acc[q - nz * pxy];
+        }
         sum += ph;
         double g = 0.0, h = 0.0;
         if (ph != 0.0) {

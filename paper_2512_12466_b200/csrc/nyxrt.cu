@@ -201,24 +201,27 @@ long long default_batch(const nyxrt_ctx *c) {
 constexpr size_t MARCH_SMEM = 0;          // the kernel's scratch is static shared memory
 
 template <int GEOM>
-void launch_march(const MarchArgs &a, bool idx64, int blocks, cudaStream_t st) {
-    if (idx64) march_kernel<GEOM, long long><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
-    else march_kernel<GEOM, int><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+void launch_march(const MarchArgs &a, bool idx64, bool per, int blocks, cudaStream_t st) {
+    if (per) {
+        if (idx64) march_kernel<GEOM, long long, true><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+        else march_kernel<GEOM, int, true><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+    } else {
+        if (idx64) march_kernel<GEOM, long long, false><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+        else march_kernel<GEOM, int, false><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+    }
+}
+
+template <typename K>
+cudaError_t setup_kernel(K kern, int *occ) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 32);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, kern, MARCH_THREADS, MARCH_SMEM);
+    return e;
 }
 
 template <int GEOM>
-cudaError_t setup_march(bool idx64, int *occ) {
-    cudaError_t e;
-    if (idx64) {
-        e = cudaFuncSetAttribute(march_kernel<GEOM, long long>, cudaFuncAttributePreferredSharedMemoryCarveout, 32);
-        if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, long long>, MARCH_THREADS, MARCH_SMEM);
-    } else {
-        e = cudaFuncSetAttribute(march_kernel<GEOM, int>, cudaFuncAttributePreferredSharedMemoryCarveout, 32);
-        if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, march_kernel<GEOM, int>, MARCH_THREADS, MARCH_SMEM);
-    }
-    return e;
+cudaError_t setup_march(bool idx64, bool per, int *occ) {
+    if (per) return idx64 ? setup_kernel(march_kernel<GEOM, long long, true>, occ) : setup_kernel(march_kernel<GEOM, int, true>, occ);
+    return idx64 ? setup_kernel(march_kernel<GEOM, long long, false>, occ) : setup_kernel(march_kernel<GEOM, int, false>, occ);
 }
 
 int geom_template(int mode) { return mode == 2 ? 3 : mode; }
@@ -227,7 +230,7 @@ int geom_template(int mode) { return mode == 2 ? 3 : mode; }
 int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     SrcBufs &s = ctx->sb;
     const long long n = ctx->n_src;
-    const GridDims gd{ctx->g.nx, ctx->g.ny, ctx->g.nz};
+    const GridDims gd{ctx->g.nx, ctx->g.ny, ctx->g.nz, ctx->g.periodic};
     ctx->n_dedup = ctx->n_cat = 0;
     ctx->cat_sel = 0;
     if (n == 0) return NYXRT_OK;
@@ -275,7 +278,7 @@ int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     tb = s.cub_bytes;
     CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.bin_a, s.bin_b, s.idx_a, s.idx_b, nd, 0, bin_bits, st));
     iota_kernel<<<nb, 256, 0, st>>>(s.par, nd);
-    link_kernel<<<nb, 256, 0, st>>>(s.cell[0], s.r[0], nd, W, nbx, nby, nbz, s.bin_b, s.idx_b, ctx->p.f_ov, ctx->p.eps,
+    link_kernel<<<nb, 256, 0, st>>>(s.cell[0], s.r[0], nd, W, nbx, nby, nbz, gd, s.bin_b, s.idx_b, ctx->p.f_ov, ctx->p.eps,
                                     s.par);
     // groups: label = smallest member; members in ascending catalogue order (stable sort by label)
     label_kernel<<<nb, 256, 0, st>>>(s.par, nd, s.lab_a, s.idx_a);
@@ -322,7 +325,7 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     if (g.nx < 1 || g.ny < 1 || g.nz < 1 || g.nx > (1 << 20) || g.ny > (1 << 20) || g.nz > (1 << 20)) return NYXRT_EINVAL;
     if ((long long)g.nx * g.ny * g.nz >= ((long long)1 << 40)) return NYXRT_EINVAL;
     if (g.field_dtype != 0 && g.field_dtype != 1) return NYXRT_EINVAL;
-    if (!(g.dx_cm > 0.0) || !(g.pos_unit_cm > 0.0) || g.periodic != 0) return NYXRT_EINVAL;
+    if (!(g.dx_cm > 0.0) || !(g.pos_unit_cm > 0.0) || (g.periodic != 0 && g.periodic != 1)) return NYXRT_EINVAL;
     if (!(p.sigma_cm2 > 0.0) || !(p.n_min_ray > 0.0) || !(p.tau_max > 0.0)) return NYXRT_EINVAL;
     if (p.level_max < 0 || p.level_max > 13 || p.geom_mode < 0 || p.geom_mode > 4) return NYXRT_EINVAL;
     if (p.merge < 0 || p.merge > 2 || p.samp_level < 0 || p.samp_level > 8 || !(p.delta_r > 0.0)) return NYXRT_EINVAL;
@@ -352,10 +355,10 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     int occ = 0;
     if (e == cudaSuccess) {
         switch (geom_template(p.geom_mode)) {
-            case 0: e = setup_march<0>(ctx->idx64, &occ); break;
-            case 1: e = setup_march<1>(ctx->idx64, &occ); break;
-            case 4: e = setup_march<4>(ctx->idx64, &occ); break;
-            default: e = setup_march<3>(ctx->idx64, &occ); break;
+            case 0: e = setup_march<0>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 1: e = setup_march<1>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 4: e = setup_march<4>(ctx->idx64, g.periodic != 0, &occ); break;
+            default: e = setup_march<3>(ctx->idx64, g.periodic != 0, &occ); break;
         }
     }
     if (e != cudaSuccess) {
@@ -426,11 +429,11 @@ int nyxrt_set_fields(nyxrt_ctx *ctx, const void *d_nH, const void *d_xHI, void *
     if (ctx->g.field_dtype)
         prep_fields_kernel<float><<<NPARTIAL, 256, 0, st>>>((const float *)d_nH, (const float *)d_xHI, ctx->absorber,
                                                             ctx->g.nx, ctx->g.ny, ctx->g.nz, ctx->p.n_th, use_flag,
-                                                            ctx->partial);
+                                                            ctx->g.periodic, ctx->partial);
     else
         prep_fields_kernel<double><<<NPARTIAL, 256, 0, st>>>((const double *)d_nH, (const double *)d_xHI, ctx->absorber,
                                                              ctx->g.nx, ctx->g.ny, ctx->g.nz, ctx->p.n_th, use_flag,
-                                                             ctx->partial);
+                                                             ctx->g.periodic, ctx->partial);
     sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 0);
     CU(cudaGetLastError());
     ctx->d_nH = d_nH;
@@ -455,7 +458,7 @@ int nyxrt_set_sources(nyxrt_ctx *ctx, int64_t n, const double *pos, const double
         CU(cudaMemcpyAsync(s.pos, pos, 3 * n * sizeof(double), cudaMemcpyHostToDevice, st));
         CU(cudaMemcpyAsync(s.L, L, n * sizeof(double), cudaMemcpyHostToDevice, st));
         CU(cudaMemsetAsync(s.bad, 0, sizeof(int), st));
-        const GridDims gd{ctx->g.nx, ctx->g.ny, ctx->g.nz};
+        const GridDims gd{ctx->g.nx, ctx->g.ny, ctx->g.nz, ctx->g.periodic};
         snap_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.pos, s.L, n, gd, ctx->g.box_lo[0], ctx->g.box_lo[1],
                                                          ctx->g.box_lo[2], ctx->g.pos_unit_cm, ctx->g.dx_cm, s.key_a,
                                                          s.bad);
@@ -516,6 +519,8 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     a.pxy = (long long)(ctx->g.nx + 2) * (ctx->g.ny + 2);
     a.sdx = ctx->p.sigma_cm2 * ctx->g.dx_cm;
     a.tau_max = ctx->p.tau_max;
+    a.s_max = std::sqrt((double)((long long)ctx->g.nx * ctx->g.nx + (long long)ctx->g.ny * ctx->g.ny +
+                                 (long long)ctx->g.nz * ctx->g.nz));       // sqrt(3) L_box for a cube
     for (int l = 0; l < MAXLEV; ++l) { a.r2_split[l] = ctx->r2_split[l]; a.K[l] = ctx->K[l]; }
     const int gt = geom_template(ctx->p.geom_mode);
     const int emit_blocks = ctx->sm_count * 4;
@@ -535,10 +540,10 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
             switch (gt) {
-                case 0: launch_march<0>(a, ctx->idx64, ctx->march_blocks, st); break;
-                case 1: launch_march<1>(a, ctx->idx64, ctx->march_blocks, st); break;
-                case 4: launch_march<4>(a, ctx->idx64, ctx->march_blocks, st); break;
-                default: launch_march<3>(a, ctx->idx64, ctx->march_blocks, st); break;
+                case 0: launch_march<0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 1: launch_march<1>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 4: launch_march<4>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                default: launch_march<3>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch + 1], st));
             ++n_launch;
@@ -553,7 +558,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     // ---- finalise ----
     const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
     finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->acc, ctx->absorber, ctx->g.nx, ctx->g.ny, ctx->g.nz, V,
-                                              ctx->p.e_excess_erg, ctx->partial);
+                                              ctx->p.e_excess_erg, ctx->g.periodic, ctx->partial);
     sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
     CU(cudaEventRecord(ctx->ev[3], st));
     CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));

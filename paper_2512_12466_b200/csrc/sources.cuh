@@ -10,7 +10,18 @@
 
 namespace nyxrt {
 
-struct GridDims { int nx, ny, nz; };
+struct GridDims { int nx, ny, nz; int periodic; };
+
+// periodic box: index into [0, n); minimum-image difference in
+// [-n/2, n/2), the tie n/2 going to -n/2 (reading R31)
+__device__ __forceinline__ long long wrap_idx(long long i, long long n) {
+    i %= n;
+    return i < 0 ? i + n : i;
+}
+__device__ __forceinline__ long long min_image(long long d, long long n) {
+    d = wrap_idx(d, n);
+    return (2 * d >= n) ? d - n : d;
+}
 
 // key = linear cell index, or -1 and *bad = 1 if the source is outside the box / L invalid (reading R2)
 __global__ void snap_kernel(const double *__restrict__ pos, const double *__restrict__ L, long long n, GridDims g,
@@ -75,10 +86,11 @@ __global__ void radius_kernel(const int4 *__restrict__ cell, long long n, const 
     while (r <= r_max) {
         int ntot = 0, nion = 0;
         for (int q = lane; q < ndir; q += 32) {
-            const long long i = c.x + (long long)floor(fma(r, dirs[3 * q], 0.5));
-            const long long j = c.y + (long long)floor(fma(r, dirs[3 * q + 1], 0.5));
-            const long long k = c.z + (long long)floor(fma(r, dirs[3 * q + 2], 0.5));
-            if (i < 0 || i >= g.nx || j < 0 || j >= g.ny || k < 0 || k >= g.nz) continue;
+            long long i = c.x + (long long)floor(fma(r, dirs[3 * q], 0.5));
+            long long j = c.y + (long long)floor(fma(r, dirs[3 * q + 1], 0.5));
+            long long k = c.z + (long long)floor(fma(r, dirs[3 * q + 2], 0.5));
+            if (g.periodic) { i = wrap_idx(i, g.nx); j = wrap_idx(j, g.ny); k = wrap_idx(k, g.nz); }
+            else if (i < 0 || i >= g.nx || j < 0 || j >= g.ny || k < 0 || k >= g.nz) continue;
             ++ntot;
             if (ion_frac(xHI, (k * g.ny + j) * g.nx + i) >= x_th) ++nion;
         }
@@ -148,28 +160,47 @@ __device__ __forceinline__ long long lower_bound_int(const int *v, long long n, 
 }
 
 // link test of Alg. 3 (PAPER.md:367-370 with the text's epsilon, 331): integer d^2, fp64 right-hand side
+// bins to search along one axis: b-1, b, b+1 inside the box; in a periodic box b-2 .. b+2 wrapped (the last
+// bin of an axis may be narrower than W, so a pair across the face can sit two bins apart), without repeats
+__device__ __forceinline__ int bin_range(int b, int nb, int periodic, int *out) {
+    int m = 0;
+    if (!periodic) {
+        for (int d = -1; d <= 1; ++d)
+            if (b + d >= 0 && b + d < nb) out[m++] = b + d;
+        return m;
+    }
+    for (int d = -2; d <= 2; ++d) {
+        const int x = (int)wrap_idx(b + d, nb);
+        bool seen = false;
+        for (int u = 0; u < m; ++u) seen = seen || out[u] == x;
+        if (!seen) out[m++] = x;
+    }
+    return m;
+}
+
 __global__ void link_kernel(const int4 *__restrict__ cell, const double *__restrict__ rad, long long n, int W,
-                            int nbx, int nby, int nbz, const int *__restrict__ sbin, const int *__restrict__ sidx,
-                            double f_ov, double eps, int *par) {
+                            int nbx, int nby, int nbz, GridDims g, const int *__restrict__ sbin,
+                            const int *__restrict__ sidx, double f_ov, double eps, int *par) {
     const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= n) return;
     const double ra = rad[a];
     if (!(ra > 0.0)) return;
     const int4 ca = cell[a];
-    const int bx = ca.x / W, by = ca.y / W, bz = ca.z / W;
-    for (int dz = -1; dz <= 1; ++dz)
-        for (int dy = -1; dy <= 1; ++dy)
-            for (int dx = -1; dx <= 1; ++dx) {
-                const int x = bx + dx, y = by + dy, z = bz + dz;
-                if (x < 0 || x >= nbx || y < 0 || y >= nby || z < 0 || z >= nbz) continue;
-                const int b = (z * nby + y) * nbx + x;
+    int lx[5], ly[5], lz[5];
+    const int mx = bin_range(ca.x / W, nbx, g.periodic, lx), my = bin_range(ca.y / W, nby, g.periodic, ly),
+              mz = bin_range(ca.z / W, nbz, g.periodic, lz);
+    for (int uz = 0; uz < mz; ++uz)
+        for (int uy = 0; uy < my; ++uy)
+            for (int ux = 0; ux < mx; ++ux) {
+                const int b = (lz[uz] * nby + ly[uy]) * nbx + lx[ux];
                 for (long long t = lower_bound_int(sbin, n, b); t < n && sbin[t] == b; ++t) {
                     const int o = sidx[t];
                     if (o <= a) continue;                                   // each pair once (a < b)
                     const double rb = rad[o];
                     if (!(rb > 0.0)) continue;
                     const int4 cb = cell[o];
-                    const long long ex = (long long)ca.x - cb.x, ey = (long long)ca.y - cb.y, ez = (long long)ca.z - cb.z;
+                    long long ex = (long long)ca.x - cb.x, ey = (long long)ca.y - cb.y, ez = (long long)ca.z - cb.z;
+                    if (g.periodic) { ex = min_image(ex, g.nx); ey = min_image(ey, g.ny); ez = min_image(ez, g.nz); }
                     const long long d2 = ex * ex + ey * ey + ez * ez;
                     const double rs = f_ov * (ra + rb);
                     if ((double)d2 <= rs * rs + eps) uf_unite(par, (int)a, o);
@@ -203,15 +234,22 @@ __global__ void collapse_kernel(const int *__restrict__ slabel, const int *__res
     const int lab = slabel[t];
     long long e = t;
     double F = 0.0, R = 0.0, n0 = 0.0, n1 = 0.0, n2 = 0.0;
+    const int4 ref = cell[sidx[t]];                // periodic: images nearest to the first member
     for (; e < n && slabel[e] == lab; ++e) {
         const int b = sidx[e];
         const double l = L[b];
         const int4 c = cell[b];
+        long long x0 = c.x, x1 = c.y, x2 = c.z;
+        if (g.periodic) {
+            x0 = ref.x + min_image(x0 - ref.x, g.nx);
+            x1 = ref.y + min_image(x1 - ref.y, g.ny);
+            x2 = ref.z + min_image(x2 - ref.z, g.nz);
+        }
         F = F + l;
         if (rad[b] > R) R = rad[b];
-        n0 = n0 + l * (double)c.x;
-        n1 = n1 + l * (double)c.y;
-        n2 = n2 + l * (double)c.z;
+        n0 = n0 + l * (double)x0;
+        n1 = n1 + l * (double)x1;
+        n2 = n2 + l * (double)x2;
     }
     int4 oc;
     double oL, oR;
@@ -219,13 +257,15 @@ __global__ void collapse_kernel(const int *__restrict__ slabel, const int *__res
         const int b = sidx[t];
         oc = cell[b]; oL = L[b]; oR = rad[b];
     } else {
-        const long long r0 = (long long)floor(n0 / F + 0.5), r1 = (long long)floor(n1 / F + 0.5),
-                        r2 = (long long)floor(n2 / F + 0.5);
+        long long r0 = (long long)floor(n0 / F + 0.5), r1 = (long long)floor(n1 / F + 0.5),
+                  r2 = (long long)floor(n2 / F + 0.5);
+        if (g.periodic) { r0 = wrap_idx(r0, g.nx); r1 = wrap_idx(r1, g.ny); r2 = wrap_idx(r2, g.nz); }
         long long bestd = -1;
         int best = -1;
         for (long long u = t; u < e; ++u) {
             const int4 c = cell[sidx[u]];
-            const long long ex = c.x - r0, ey = c.y - r1, ez = c.z - r2;
+            long long ex = c.x - r0, ey = c.y - r1, ez = c.z - r2;
+            if (g.periodic) { ex = min_image(ex, g.nx); ey = min_image(ey, g.ny); ez = min_image(ez, g.nz); }
             const long long d2 = ex * ex + ey * ey + ez * ez;
             if (best < 0 || d2 < bestd) { best = sidx[u]; bestd = d2; }
         }

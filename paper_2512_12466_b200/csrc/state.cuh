@@ -52,7 +52,8 @@ constexpr int FETCH_CHUNK = 32;          // rays a warp claims per atomic (small
 
 struct MarchArgs {
     const double *absorber;              // PADDED grid (nx+2)(ny+2)(nz+2): |a| = n_H x_HI; sign bit set where
-                                         // n_H < n_th (Eq. 7-8 flag); halo = -inf (outside the box)
+                                         // n_H < n_th (Eq. 7-8 flag); halo = -inf (outside the box), or the
+                                         // wrapped image of the opposite side in a periodic box
     double *acc;                         // PADDED: photons absorbed per cell
     const int4 *cat_cell;                // (i, j, k, 0) per catalogue source
     const double *cat_L;
@@ -63,6 +64,8 @@ struct MarchArgs {
     long long px, pxy;                   // padded strides: px = nx+2, pxy = (nx+2)(ny+2)
     double sdx;                          // sigma * dx: optical depth per unit absorber per cell length
     double tau_max;
+    double s_max;                        // periodic box: a ray ends once its travel distance s >= sqrt(nx^2+ny^2+nz^2)
+                                         // cells = sqrt(3) L_box for a cube
     double r2_split[MAXLEV];             // Eq. 4: split when s^2 > 3 4^l / (pi N_min)
     double K[MAXLEV];                    // sqrt(Omega(l)) = sqrt(pi/3) 2^-l: L_pix = R K
 };

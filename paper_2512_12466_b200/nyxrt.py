@@ -185,14 +185,15 @@ def nyxrt_destroy(ctx):
 
 # ---- small convenience wrapper used by tests / bench (still marshalling only) --------------------------
 
-def make_grid(shape_zyx, dx_cm, field_dtype=torch.float64, box_lo=(0.0, 0.0, 0.0), pos_unit_cm=None, device=0):
+def make_grid(shape_zyx, dx_cm, field_dtype=torch.float64, box_lo=(0.0, 0.0, 0.0), pos_unit_cm=None, device=0,
+              periodic=0):
     g = nyxrt_grid()
     g.nz, g.ny, g.nx = [int(v) for v in shape_zyx]
     g.field_dtype = 1 if field_dtype == torch.float32 else 0
     g.dx_cm = float(dx_cm)
     g.box_lo[:] = [float(v) for v in box_lo]
     g.pos_unit_cm = float(dx_cm if pos_unit_cm is None else pos_unit_cm)
-    g.periodic = 0
+    g.periodic = int(periodic)
     g.device = int(device)
     return g
 
@@ -208,10 +209,10 @@ class Tracer:
     """Owns a context and its torch-allocated workspace."""
 
     def __init__(self, shape_zyx, dx_cm, params, field_dtype=torch.float64, max_sources=1, batch_rays=0,
-                 host_staging=False, device=0):
+                 host_staging=False, device=0, periodic=0):
         if not torch.cuda.is_available():
             raise RuntimeError("nyxrt needs a CUDA device; there is no CPU fallback")
-        self.grid = make_grid(shape_zyx, dx_cm, field_dtype, device=device)
+        self.grid = make_grid(shape_zyx, dx_cm, field_dtype, device=device, periodic=periodic)
         self.params = make_params(**params)
         self.shape = tuple(int(v) for v in shape_zyx)
         self.device = torch.device("cuda", device)

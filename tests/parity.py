@@ -21,15 +21,15 @@ def oracle_inputs(cfg):
     return nH, xHI, cfg["src_pos"].numpy(), cfg["src_L"].numpy()
 
 
-def run_oracle(O, cfg, params=None):
+def run_oracle(O, cfg, params=None, periodic=0):
     p = dict(cfg["params"])
     p.update(params or {})
     nH, xHI, pos, L = oracle_inputs(cfg)
-    g = O.make_grid(cfg["shape"], cfg["dx_cm"], field_dtype=nH.dtype)
+    g = O.make_grid(cfg["shape"], cfg["dx_cm"], field_dtype=nH.dtype, periodic=periodic)
     return O.step(g, O.make_params(**p), nH, xHI, pos, L)
 
 
-def run_gpu(cfg, params=None, batch_rays=0, want_heat=True, host=False):
+def run_gpu(cfg, params=None, batch_rays=0, want_heat=True, host=False, periodic=0):
     from paper_2512_12466_b200 import nyxrt
     p = dict(cfg["params"])
     p.update(params or {})
@@ -37,7 +37,7 @@ def run_gpu(cfg, params=None, batch_rays=0, want_heat=True, host=False):
     xHI = cfg["xHI"].cuda().contiguous()
     pos, L = cfg["src_pos"].numpy(), cfg["src_L"].numpy()
     tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], p, field_dtype=nH.dtype, max_sources=len(L),
-                      batch_rays=batch_rays, host_staging=host)
+                      batch_rays=batch_rays, host_staging=host, periodic=periodic)
     try:
         if host:
             gam = torch.empty(cfg["shape"], dtype=torch.float64).pin_memory()

@@ -192,6 +192,6 @@ def test_error_paths():
     assert e.value.code == nyxrt.ESTATE
     tr.close()
     bad = nyxrt.make_grid((16, 16, 16), 1e20)
-    bad.periodic = 1
+    bad.periodic = 2
     with pytest.raises(nyxrt.NyxrtError):
         nyxrt.nyxrt_create(bad, nyxrt.make_params(**p))
