@@ -650,3 +650,106 @@ int orc_step(const orc_grid *g, const orc_params *p, const void *nH, const void 
 
 int orc_sizeof_stats(void) { return (int)sizeof(orc_stats); }
 int orc_sizeof_seg(void) { return (int)sizeof(orc_seg); }
+
+/* ------------------------------------------------------------------------------------------ */
+/* T1-T3: one RT TIMESTEP = time integration (Sec. 2.3) inside the iterative     */
+/* nonlinear solve (Sec. 2.4), "following the approach of [23]" (C2-Ray,        */
+/* Mellema et al. 2006): fix x, ray-trace for Gamma (orc_step above); fix Gamma, integrate Eq. 3  */
+/* over dt with the semi-analytic, time-averaged solution; iterate until convergence.             */
+/* Monochromatic (constant sigma): the frequency-integrated lookup table of PAPER.md:95 is not    */
+/* built (the paper prints no source spectrum).  Readings R32-R36.                    */
+
+typedef struct {
+    double  dt_s;             /* timestep                                                       */
+    double  alpha_cm3_s;      /* recombination coefficient alpha_H(T) of Eq. 3 (isothermal, caller's T) */
+    double  coll_cm3_s;       /* collisional ionisation coefficient C_H(T) of Eq. 3              */
+    double  clumping;         /* clumping factor C of Eq. 10 (multiplies the recombination rate) */
+    double  tol_rel, tol_abs; /* convergence of the time-averaged neutral fraction (R35)         */
+    double  unconv_frac;      /* fraction of the cells that may stay unconverged (R35)           */
+    int32_t max_iter;         /* outer iterations (RT <-> ODE), >= 1                             */
+    int32_t inner_iter;       /* per-cell iterations on the electron density, >= 1 (R34)         */
+} orc_ode;
+
+typedef struct {
+    int32_t  iterations, converged;
+    uint64_t unconverged_cells;    /* in the last iteration                                      */
+    uint64_t segments_total;       /* over all iterations                                        */
+    double   max_rel_change;       /* of the last iteration: max |dy| / (tol_rel y + tol_abs)    */
+} orc_tstats;
+
+/* T2: Eq. 3 in one cell with Gamma fixed, written for the NEUTRAL fraction y = 1 - x:
+       dy/dt = -y (Gamma + n_e C_H) + (1 - y) n_e alpha_H C  =  a_rec - y (a_ion + a_rec),
+   n_e = <x> n_H held at its time average ([23]'s "time averaging"; the paper's
+   "n_e = x n_HI" is read as x n_H, R33).  With constant coefficients the solution is
+       y(t) = y_eq + (y0 - y_eq) e^{-t/t_i},  t_i = 1/(a_ion + a_rec),  y_eq = a_rec t_i,
+       <y>  = y_eq + (y0 - y_eq) (1 - e^{-dt/t_i}) t_i/dt.
+   <y> feeds n_e again, inner_iter times (R34).  yavg_io: in = the current estimate of <y>. */
+void orc_ode_cell(const orc_ode *o, double gamma, double nH, double y0, double *yavg_io, double *yend_out) {
+    double yavg = *yavg_io, yend = y0;
+    for (int it = 0; it < o->inner_iter; ++it) {
+        double ne = (1.0 - yavg) * nH;
+        double a_ion = gamma + ne * o->coll_cm3_s;
+        double a_rec = (ne * o->alpha_cm3_s) * o->clumping;
+        double rate = a_ion + a_rec;
+        double w = rate * o->dt_s;
+        if (!(w > 0.0)) { yend = y0; yavg = y0; break; }           /* nothing acts on the cell */
+        double yeq = a_rec / rate;
+        double em1 = expm1(-w);                                      /* e^{-w} - 1 */
+        yend = yeq + (y0 - yeq) * (1.0 + em1);
+        yavg = yeq + (y0 - yeq) * (-em1 / w);
+        if (yend < 0.0) yend = 0.0;
+        if (yend > 1.0) yend = 1.0;
+        if (yavg < 0.0) yavg = 0.0;
+        if (yavg > 1.0) yavg = 1.0;
+    }
+    *yavg_io = yavg;
+    *yend_out = yend;
+}
+
+/* T3: the iterative solve.  xHI_begin: neutral fraction at the start of the step (fp64).
+   xHI_avg: work / output in the FIELD dtype (it is the x_HI field of every ray trace; R36: the
+   first trace uses the neutral fraction at the start of the step).  xHI_end: fp64 output.
+   gamma / heat: the last iteration's rates.  st: the last iteration's ray statistics. */
+int orc_timestep(const orc_grid *g, const orc_params *p, const orc_ode *o, const void *nH,
+                 const double *xHI_begin, int64_t n_src, const double *pos, const double *L,
+                 double *xHI_end, void *xHI_avg, double *gamma, double *heat, orc_stats *st,
+                 orc_tstats *ts, int32_t *cat_cell, double *cat_L, double *cat_r, int64_t *n_cat) {
+    if (!(o->dt_s > 0.0) || o->max_iter < 1 || o->inner_iter < 1 || !(o->alpha_cm3_s >= 0.0) ||
+        !(o->coll_cm3_s >= 0.0) || !(o->clumping >= 0.0) || !(o->tol_rel >= 0.0) || !(o->tol_abs >= 0.0) || !(o->unconv_frac >= 0.0))
+        return ORC_EINVAL;
+    const int64_t ncell = (int64_t)g->nx * g->ny * g->nz;
+    memset(ts, 0, sizeof *ts);
+    for (int64_t c = 0; c < ncell; ++c) {
+        if (g->field_dtype) ((float *)xHI_avg)[c] = (float)xHI_begin[c];
+        else ((double *)xHI_avg)[c] = xHI_begin[c];
+    }
+    for (int it = 0; it < o->max_iter; ++it) {
+        int rc = orc_step(g, p, nH, xHI_avg, n_src, pos, L, gamma, heat, st, cat_cell, cat_L, cat_r, n_cat);
+        if (rc) return rc;
+        ts->iterations = it + 1;
+        ts->segments_total += st->segments;
+        uint64_t bad = 0;
+        double worst = 0.0;
+        for (int64_t c = 0; c < ncell; ++c) {
+            double y_old = fld(xHI_avg, g->field_dtype, c);
+            double yavg = y_old, yend;
+            orc_ode_cell(o, gamma[c], fld(nH, g->field_dtype, c), xHI_begin[c], &yavg, &yend);
+            double y_new;
+            if (g->field_dtype) { ((float *)xHI_avg)[c] = (float)yavg; y_new = (double)(float)yavg; }
+            else { ((double *)xHI_avg)[c] = yavg; y_new = yavg; }
+            xHI_end[c] = yend;
+            double lim = o->tol_rel * y_new + o->tol_abs;            /* R35 */
+            double dy = fabs(y_new - y_old);
+            if (dy > lim) ++bad;
+            double q = lim > 0.0 ? dy / lim : (dy > 0.0 ? INFINITY : 0.0);
+            if (q > worst) worst = q;
+        }
+        ts->unconverged_cells = bad;
+        ts->max_rel_change = worst;
+        if ((double)bad <= o->unconv_frac * (double)ncell) { ts->converged = 1; break; }
+    }
+    return ORC_OK;
+}
+
+int orc_sizeof_ode(void) { return (int)sizeof(orc_ode); }
+int orc_sizeof_tstats(void) { return (int)sizeof(orc_tstats); }

@@ -211,3 +211,64 @@ def step(g, p, nH, xHI, pos, L, want_heat=True):
 
 def mean_ionised(g, xHI):
     return lib().orc_mean_ionised(C.byref(g), _ptr(_field(g, xHI)))
+
+
+# ---- RT timestep: time integration + iterative solve (following [23]) ---------------
+
+class Ode(C.Structure):
+    _fields_ = [("dt_s", C.c_double), ("alpha_cm3_s", C.c_double), ("coll_cm3_s", C.c_double),
+                ("clumping", C.c_double), ("tol_rel", C.c_double), ("tol_abs", C.c_double),
+                ("unconv_frac", C.c_double),
+                ("max_iter", C.c_int32), ("inner_iter", C.c_int32)]
+
+
+class TStats(C.Structure):
+    _fields_ = [("iterations", C.c_int32), ("converged", C.c_int32), ("unconverged_cells", C.c_uint64),
+                ("segments_total", C.c_uint64), ("max_rel_change", C.c_double)]
+
+
+def make_ode(dt_s, **kw):
+    """Defaults: DESIGN.md "Parameters" (alpha_B(1e4 K) = 2.59e-13)."""
+    d = dict(alpha_cm3_s=2.59e-13, coll_cm3_s=0.0, clumping=1.0, tol_rel=1e-2, tol_abs=1e-5, unconv_frac=1e-4,
+             max_iter=30, inner_iter=8)
+    d.update(kw)
+    o = Ode()
+    o.dt_s = float(dt_s)
+    for k, v in d.items():
+        setattr(o, k, v)
+    assert lib().orc_sizeof_ode() == C.sizeof(Ode) and lib().orc_sizeof_tstats() == C.sizeof(TStats)
+    return o
+
+
+def ode_cell(o, gamma, nH, y0, yavg):
+    """One cell of T2.  Returns (y_avg, y_end)."""
+    ya, ye = C.c_double(yavg), C.c_double(0.0)
+    f = lib().orc_ode_cell
+    f.restype = None
+    f(C.byref(o), C.c_double(gamma), C.c_double(nH), C.c_double(y0), C.byref(ya), C.byref(ye))
+    return ya.value, ye.value
+
+
+def timestep(g, p, o, nH, xHI_begin, pos, L, want_heat=True):
+    """One RT timestep.  Returns (xHI_end f64, xHI_avg field dtype, gamma, heat, stats, tstats, catalogue)."""
+    nH = _field(g, nH)
+    xb = np.ascontiguousarray(xHI_begin, dtype=np.float64)
+    assert xb.shape == (g.nz, g.ny, g.nx)
+    pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+    L = np.ascontiguousarray(L, dtype=np.float64)
+    n = len(L)
+    shape = (g.nz, g.ny, g.nx)
+    xe = np.zeros(shape)
+    xa = np.zeros(shape, np.float32 if g.field_dtype else np.float64)
+    gamma = np.zeros(shape)
+    heat = np.zeros(shape) if want_heat else None
+    st, ts = Stats(), TStats()
+    cc = np.zeros((max(n, 1), 3), np.int32)
+    cL = np.zeros(max(n, 1))
+    cr = np.zeros(max(n, 1))
+    ncat = C.c_int64(0)
+    _chk(lib().orc_timestep(C.byref(g), C.byref(p), C.byref(o), _ptr(nH), _ptr(xb), C.c_int64(n), _ptr(pos), _ptr(L),
+                            _ptr(xe), _ptr(xa), _ptr(gamma), _ptr(heat) if want_heat else None, C.byref(st),
+                            C.byref(ts), _ptr(cc), _ptr(cL), _ptr(cr), C.byref(ncat)), "timestep")
+    m = ncat.value
+    return xe, xa, gamma, heat, st, ts, (cc[:m].copy(), cL[:m].copy(), cr[:m].copy())
