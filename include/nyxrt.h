@@ -154,6 +154,42 @@ int nyxrt_get_catalog(nyxrt_ctx *ctx, int64_t cap, int32_t *cell_ijk, double *L,
 int nyxrt_step_host(nyxrt_ctx *ctx, const void *h_nH, const void *h_xHI, int64_t n_src, const double *pos_xyz,
                     const double *L, double *h_gamma_HI, double *h_heat, nyxrt_stats *h_stats);
 
+/* Parameters of one RT TIMESTEP (time integration, Eq. 3, inside the iterative nonlinear
+ * solve, "following [23]"; monochromatic, the lookup table of PAPER.md:95 is not built). */
+typedef struct {
+    double  dt_s;              /* timestep [s], > 0                                                  */
+    double  alpha_cm3_s;       /* recombination coefficient alpha_H(T) of Eq. 3 (2.59e-13 at 1e4 K)  */
+    double  coll_cm3_s;        /* collisional ionisation coefficient C_H(T) of Eq. 3                 */
+    double  clumping;          /* clumping factor C of Eq. 10: multiplies the recombination rate     */
+    double  tol_rel, tol_abs;  /* a cell has converged when |d<x_HI>| <= tol_rel <x_HI> + tol_abs (R35) */
+    double  unconv_frac;       /* fraction of the cells that may stay unconverged (R35)              */
+    int32_t max_iter;          /* ray trace <-> update iterations, >= 1                              */
+    int32_t inner_iter;        /* per-cell iterations on the electron density, >= 1 (R34)            */
+} nyxrt_ode;
+
+typedef struct {
+    int32_t  iterations, converged;
+    uint64_t unconverged_cells;          /* in the last iteration                                    */
+    uint64_t segments_total;             /* ray-cell segments over all iterations                    */
+    uint64_t kernel_launches;            /* own kernels over all iterations                          */
+    double   max_rel_change;             /* last iteration: max |d<x_HI>| / (tol_rel <x_HI> + tol_abs) */
+    float    ms_total, ms_rt, ms_ode, pad_;
+} nyxrt_tstats;
+
+/* One RT timestep of length ode->dt_s: starting from the neutral fraction d_xHI_begin (fp64, [nz][ny][nx]),
+ * iterate { nyxrt_set_fields(d_nH, d_xHI_avg); nyxrt_trace -> Gamma; per cell, integrate Eq. 3 over dt with
+ * Gamma fixed and n_e at its time average (semi-analytic, time-averaged solution of [23]) -> x_HI at the end
+ * of the step and its time average } until the time-averaged neutral fraction stops changing or max_iter.
+ * All pointers are device pointers.  d_nH: grid.field_dtype.  d_xHI_avg: grid.field_dtype, written (the x_HI
+ * field of every ray trace; on return the converged time average, and the registered field of the context).
+ * d_xHI_end: fp64, written.  d_gamma_HI / d_heat (may be NULL): the last iteration's rates.  h_stats (may be
+ * NULL): the last ray trace's statistics.  h_tstats (may be NULL).  Sources must have been set.  Synchronises
+ * `stream` every iteration (the convergence test is read on the host).
+ * Errors: EINVAL (NULL, bad parameters), ESTATE (workspace / sources missing), EOVERFLOW, ECUDA. */
+int nyxrt_timestep(nyxrt_ctx *ctx, const nyxrt_ode *ode, const void *d_nH, const double *d_xHI_begin,
+                   double *d_xHI_end, void *d_xHI_avg, double *d_gamma_HI, double *d_heat, nyxrt_stats *h_stats,
+                   nyxrt_tstats *h_tstats, void *cuda_stream);
+
 /* HEALPix nested pixel centre of (level, pix) as the library computes it on the device (DIR-SPEC,
  * DESIGN.md): n directions into the host array dir_xyz [n][3].  For tests.  Errors: EINVAL, ECUDA. */
 int nyxrt_pix2dir(nyxrt_ctx *ctx, int32_t level, int64_t pix_begin, int64_t n, double *dir_xyz);
@@ -169,6 +205,8 @@ int nyxrt_version(void);
 int nyxrt_sizeof_grid(void);
 int nyxrt_sizeof_params(void);
 int nyxrt_sizeof_stats(void);
+int nyxrt_sizeof_ode(void);
+int nyxrt_sizeof_tstats(void);
 
 #ifdef __cplusplus
 }

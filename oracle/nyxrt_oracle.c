@@ -3,7 +3,7 @@
  *
  * A plain, slow, single-threaded fp64 CPU statement of ONE adaptive ray-tracing step on a
  * uniform coarse grid, written from the paper (arxiv 2512.12466, text at
- * /root/reference/PAPER.md; "PAPER.md:<line>" below) with the readings R1..R27 recorded in
+ * /root/reference/PAPER.md; "PAPER.md:<line>" below) with the readings R1..R36 recorded in
  * DESIGN.md ("Readings").  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference leg may load this file.  It shares no code, header, table or helper with the
  * CUDA library under paper_2512_12466_b200/csrc and neither includes the other.
@@ -17,6 +17,8 @@
  *                         depth-first until no ray is left                  (PAPER.md:111-128,
  *                         152-199, 83-95 Eq. 1-2, 211-249 Eq. 5-8)
  *   orc_step              the four above in order.
+ *   orc_timestep          orc_step inside the iterative RT <-> ODE solve with the time-averaged update
+ *                         of Eq. 3 (orc_ode_cell)                          ([23])
  *
  * Traversal is depth-first and recursive (a split recurses into the four children), which is
  * structurally unlike the CUDA library's pooled breadth-first loop.

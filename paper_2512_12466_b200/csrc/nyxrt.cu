@@ -17,6 +17,7 @@
 #include "../../include/nyxrt.h"
 #include "march.cuh"
 #include "sources.cuh"
+#include "timestep.cuh"
 
 using namespace nyxrt;
 
@@ -70,6 +71,7 @@ struct nyxrt_ctx {
     int cat_sel;                           // which of sb.cell[]/L2[]/r[] holds the final catalogue
     double r2_split[MAXLEV], K[MAXLEV];
     cudaEvent_t ev[4];
+    cudaEvent_t tev[4];                    // timestep phases
     cudaEvent_t *mev;                      // pairs of events around every march launch
     long long mev_cap;
     cudaStream_t own_stream;
@@ -314,6 +316,8 @@ int nyxrt_version(void) { return 100; }
 int nyxrt_sizeof_grid(void) { return (int)sizeof(nyxrt_grid); }
 int nyxrt_sizeof_params(void) { return (int)sizeof(nyxrt_params); }
 int nyxrt_sizeof_stats(void) { return (int)sizeof(nyxrt_stats); }
+int nyxrt_sizeof_ode(void) { return (int)sizeof(nyxrt_ode); }
+int nyxrt_sizeof_tstats(void) { return (int)sizeof(nyxrt_tstats); }
 
 const char *nyxrt_last_error(const nyxrt_ctx *ctx) { return ctx ? ctx->err : "null context"; }
 
@@ -349,6 +353,7 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, g.device);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking);
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev[k]);
+    for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->tev[k]);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ls, sizeof(LoopState));
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ds, sizeof(DevStats));
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_scalars, 8 * sizeof(double));
@@ -379,6 +384,8 @@ void nyxrt_destroy(nyxrt_ctx *ctx) {
     free(ctx->mev);
     for (int k = 0; k < 4; ++k)
         if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+    for (int k = 0; k < 4; ++k)
+        if (ctx->tev[k]) cudaEventDestroy(ctx->tev[k]);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->h_ls) cudaFreeHost(ctx->h_ls);
     if (ctx->h_ds) cudaFreeHost(ctx->h_ds);
@@ -645,6 +652,68 @@ int nyxrt_step_host(nyxrt_ctx *ctx, const void *h_nH, const void *h_xHI, int64_t
     CU(cudaMemcpyAsync(h_gamma, ctx->st_gamma, ctx->ncell * sizeof(double), cudaMemcpyDeviceToHost, st));
     if (h_heat) CU(cudaMemcpyAsync(h_heat, ctx->st_heat, ctx->ncell * sizeof(double), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    return NYXRT_OK;
+}
+
+int nyxrt_timestep(nyxrt_ctx *ctx, const nyxrt_ode *ode, const void *d_nH, const double *d_y_begin, double *d_y_end,
+                   void *d_y_avg, double *d_gamma, double *d_heat, nyxrt_stats *hs, nyxrt_tstats *ht, void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!ode || !d_nH || !d_y_begin || !d_y_end || !d_y_avg || !d_gamma)
+        return fail(ctx, NYXRT_EINVAL, "timestep: null pointer");
+    const nyxrt_ode &o = *ode;
+    if (!(o.dt_s > 0.0) || o.max_iter < 1 || o.inner_iter < 1 || !(o.alpha_cm3_s >= 0.0) || !(o.coll_cm3_s >= 0.0) ||
+        !(o.clumping >= 0.0) || !(o.tol_rel >= 0.0) || !(o.tol_abs >= 0.0) || !(o.unconv_frac >= 0.0))
+        return fail(ctx, NYXRT_EINVAL, "timestep: bad parameters");
+    if (!ctx->ws || !ctx->have_sources) return fail(ctx, NYXRT_ESTATE, "timestep: workspace and sources must be set first");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->g.device));
+    const long long n = ctx->ncell;
+    const bool f32 = ctx->g.field_dtype != 0;
+    const OdeArgs oa{o.dt_s, o.alpha_cm3_s, o.coll_cm3_s, o.clumping, o.tol_rel, o.tol_abs, o.inner_iter};
+    unsigned long long *conv = reinterpret_cast<unsigned long long *>(ctx->scalars + 4);
+    nyxrt_tstats t;
+    memset(&t, 0, sizeof t);
+    nyxrt_stats s_last;
+    memset(&s_last, 0, sizeof s_last);
+    cudaEvent_t e0 = ctx->tev[0], e1 = ctx->tev[1], e2 = ctx->tev[2], e3 = ctx->tev[3];
+    CU(cudaEventRecord(e0, st));
+    if (f32) init_avg_kernel<float><<<NPARTIAL, 256, 0, st>>>(d_y_begin, (float *)d_y_avg, n);
+    else init_avg_kernel<double><<<NPARTIAL, 256, 0, st>>>(d_y_begin, (double *)d_y_avg, n);
+    t.kernel_launches = 1;
+    double ms_rt = 0.0, ms_ode = 0.0;
+    for (int it = 0; it < o.max_iter; ++it) {
+        int rc = nyxrt_set_fields(ctx, d_nH, d_y_avg, st);
+        if (rc) return rc;
+        rc = nyxrt_trace(ctx, d_gamma, d_heat, &s_last, st);
+        if (rc) return rc;
+        t.iterations = it + 1;
+        t.segments_total += s_last.segments;
+        t.kernel_launches += s_last.kernel_launches + 2 + 1;          // + prep_fields, sum_partials, ode
+        ms_rt += s_last.ms_total;
+        CU(cudaEventRecord(e1, st));
+        CU(cudaMemsetAsync(conv, 0, 2 * sizeof(unsigned long long), st));
+        if (f32) ode_kernel<float><<<NPARTIAL, 256, 0, st>>>(d_gamma, (const float *)d_nH, d_y_begin, (float *)d_y_avg, d_y_end, n, oa, conv);
+        else ode_kernel<double><<<NPARTIAL, 256, 0, st>>>(d_gamma, (const double *)d_nH, d_y_begin, (double *)d_y_avg, d_y_end, n, oa, conv);
+        CU(cudaEventRecord(e2, st));
+        CU(cudaMemcpyAsync(ctx->h_scalars + 4, conv, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        CU(cudaGetLastError());
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e1, e2);
+        ms_ode += ms;
+        unsigned long long hv[2];
+        memcpy(hv, ctx->h_scalars + 4, sizeof hv);
+        t.unconverged_cells = hv[0];
+        memcpy(&t.max_rel_change, &hv[1], sizeof(double));
+        if ((double)hv[0] <= o.unconv_frac * (double)n) { t.converged = 1; break; }
+    }
+    CU(cudaEventRecord(e3, st));
+    CU(cudaEventSynchronize(e3));
+    cudaEventElapsedTime(&t.ms_total, e0, e3);
+    t.ms_rt = (float)ms_rt;
+    t.ms_ode = (float)ms_ode;
+    if (hs) *hs = s_last;
+    if (ht) *ht = t;
     return NYXRT_OK;
 }
 

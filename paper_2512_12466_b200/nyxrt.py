@@ -58,9 +58,22 @@ class nyxrt_stats(C.Structure):
         return d
 
 
+class nyxrt_ode(C.Structure):
+    _fields_ = [("dt_s", C.c_double), ("alpha_cm3_s", C.c_double), ("coll_cm3_s", C.c_double),
+                ("clumping", C.c_double), ("tol_rel", C.c_double), ("tol_abs", C.c_double),
+                ("unconv_frac", C.c_double), ("max_iter", C.c_int32), ("inner_iter", C.c_int32)]
+
+
+class nyxrt_tstats(C.Structure):
+    _fields_ = [("iterations", C.c_int32), ("converged", C.c_int32), ("unconverged_cells", C.c_uint64),
+                ("segments_total", C.c_uint64), ("kernel_launches", C.c_uint64), ("max_rel_change", C.c_double),
+                ("ms_total", C.c_float), ("ms_rt", C.c_float), ("ms_ode", C.c_float), ("pad_", C.c_float)]
+
+
 EXPORTS = ["nyxrt_create", "nyxrt_workspace_bytes", "nyxrt_set_workspace", "nyxrt_set_fields", "nyxrt_set_sources",
            "nyxrt_trace", "nyxrt_get_catalog", "nyxrt_step_host", "nyxrt_pix2dir", "nyxrt_last_error",
-           "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats"]
+           "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats",
+           "nyxrt_timestep", "nyxrt_sizeof_ode", "nyxrt_sizeof_tstats"]
 
 _lib = None
 
@@ -83,6 +96,8 @@ def lib():
         assert L.nyxrt_sizeof_grid() == C.sizeof(nyxrt_grid)
         assert L.nyxrt_sizeof_params() == C.sizeof(nyxrt_params)
         assert L.nyxrt_sizeof_stats() == C.sizeof(nyxrt_stats)
+        assert L.nyxrt_sizeof_ode() == C.sizeof(nyxrt_ode)
+        assert L.nyxrt_sizeof_tstats() == C.sizeof(nyxrt_tstats)
         _lib = L
     return _lib
 
@@ -146,6 +161,21 @@ def nyxrt_trace(ctx, gamma, heat=None, stream=None):
     return st
 
 
+def nyxrt_timestep(ctx, ode, nH, xHI_begin, xHI_end, xHI_avg, gamma, heat=None, stream=None):
+    """One RT timestep; all arrays are CUDA tensors (xHI_begin / xHI_end / gamma / heat fp64, nH / xHI_avg of the
+    field dtype).  Returns (stats of the last ray trace, timestep stats)."""
+    for t in (nH, xHI_begin, xHI_end, xHI_avg, gamma) + ((heat,) if heat is not None else ()):
+        assert t.is_cuda and t.is_contiguous()
+    assert xHI_begin.dtype == xHI_end.dtype == gamma.dtype == torch.float64 and nH.dtype == xHI_avg.dtype
+    st, ts = nyxrt_stats(), nyxrt_tstats()
+    _check(ctx, lib().nyxrt_timestep(ctx, C.byref(ode), C.c_void_p(nH.data_ptr()), C.c_void_p(xHI_begin.data_ptr()),
+                                     C.c_void_p(xHI_end.data_ptr()), C.c_void_p(xHI_avg.data_ptr()),
+                                     C.c_void_p(gamma.data_ptr()),
+                                     C.c_void_p(heat.data_ptr()) if heat is not None else None,
+                                     C.byref(st), C.byref(ts), _stream_ptr(stream)))
+    return st, ts
+
+
 def nyxrt_get_catalog(ctx):
     n = C.c_int64(0)
     _check(ctx, lib().nyxrt_get_catalog(ctx, C.c_int64(0), None, None, None, C.byref(n)))
@@ -198,6 +228,18 @@ def make_grid(shape_zyx, dx_cm, field_dtype=torch.float64, box_lo=(0.0, 0.0, 0.0
     return g
 
 
+def make_ode(dt_s, **kw):
+    """Defaults: DESIGN.md "Parameters" (alpha_B(1e4 K) = 2.59e-13 cm^3/s)."""
+    d = dict(alpha_cm3_s=2.59e-13, coll_cm3_s=0.0, clumping=1.0, tol_rel=1e-2, tol_abs=1e-5, unconv_frac=1e-4,
+             max_iter=30, inner_iter=8)
+    d.update(kw)
+    o = nyxrt_ode()
+    o.dt_s = float(dt_s)
+    for k, v in d.items():
+        setattr(o, k, v)
+    return o
+
+
 def make_params(**kw):
     p = nyxrt_params()
     for k, v in kw.items():
@@ -236,6 +278,16 @@ class Tracer:
             heat = torch.empty(self.shape, dtype=torch.float64, device=self.device)
         st = nyxrt_trace(self.ctx, gamma, heat, stream)
         return gamma, heat, st
+
+    def timestep(self, ode, nH, xHI_begin, want_heat=True, stream=None):
+        """Returns (xHI_end, xHI_avg, gamma, heat, stats, tstats); the sources must have been set."""
+        xe = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        xa = torch.empty(self.shape, dtype=nH.dtype, device=self.device)
+        gamma = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        heat = torch.empty(self.shape, dtype=torch.float64, device=self.device) if want_heat else None
+        self._fields = (nH, xa)
+        st, ts = nyxrt_timestep(self.ctx, ode, nH, xHI_begin, xe, xa, gamma, heat, stream)
+        return xe, xa, gamma, heat, st, ts
 
     def catalog(self):
         return nyxrt_get_catalog(self.ctx)
