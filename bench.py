@@ -34,6 +34,8 @@ def parse():
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--n-src", type=int, default=0, help="use only the first N sources (0 = all)")
     ap.add_argument("--batch-rays", type=int, default=0)
+    ap.add_argument("--shard", action="store_true",
+                    help="N > 1: shard the step by source (one all-reduce of the photon grid) instead of N replicas")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -102,6 +104,16 @@ def max_over_ranks(x, device):
     t = torch.tensor([float(x)], dtype=torch.float64, device=device)
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x, device):
+    """Sum of a scalar over all ranks (source-sharded mode: every rank marches its own rays)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return float(t.item())
 
 
@@ -205,11 +217,22 @@ def main():
     heat = torch.empty_like(gam)
     stream = torch.cuda.current_stream()
 
+    photons = torch.empty_like(gam) if args.shard else None
+    if args.shard:
+        tr.set_shard(rank, world)
+
     def step():
         # one RT step: fields of this step -> absorber field, sources -> catalogue, ray loop, finalise
         tr.set_fields(nH, xHI, stream)
         tr.set_sources(pos, L, stream)
-        return tr.trace(gam, heat, stream=stream)[2]
+        if not args.shard:
+            return tr.trace(gam, heat, stream=stream)[2]
+        # sharded by source: this rank's sources, one all-reduce of the photon grid
+        st_ = nyxrt.nyxrt_trace_photons(tr.ctx, photons, stream)
+        if world > 1:
+            dist.all_reduce(photons, op=dist.ReduceOp.SUM)
+        nyxrt.nyxrt_finalise(tr.ctx, photons, gam, heat, stream)
+        return st_
 
     for _ in range(args.warmup):
         st = step()
@@ -235,7 +258,13 @@ def main():
     ms = e0.elapsed_time(e1)
     clk = clocks.stop() if rank == 0 else None
     ms = max_over_ranks(ms, "cuda")
-    value = whole_job_rate(seg, ms, world)
+    if args.shard:
+        seg_all = sum_over_ranks(seg, "cuda")                       # total work is fixed: strong scaling
+        value = whole_job_rate(seg_all, ms, 1)
+        args.no_e2e = True                                          # step_host is the unsharded call
+    else:
+        seg_all = seg * world
+        value = whole_job_rate(seg, ms, world)
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
     e2e = None
@@ -281,14 +310,14 @@ def main():
             cpu = oracle_sample(cfg, pos, L, args.cpu_seconds)
             cpu.pop("segments"); cpu.pop("seconds")
         out = dict(metric=METRIC, value=value, unit="segments/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
-                   ms_per_step=ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
-                   data="synthetic",
+                   ms_per_step=ms / args.steps, higher_is_better=True, scaling="strong" if args.shard else "weak",
+                   vs_baseline=None, dtype="f64", data="synthetic",
                    config=dict(workload=cfg["name"], grid=list(cfg["shape"]), field_dtype=fdt, n_sources=int(len(L)),
                                n_sources_dedup=int(st.n_src_dedup), n_sources_merged=int(st.n_src_merged),
-                               segments_per_step=int(seg // args.steps), notes=cfg["notes"],
+                               segments_per_step=int(seg_all // (args.steps * (1 if args.shard else world))), notes=cfg["notes"],
                                l2="inputs larger than L2 (fields + accumulator = %.1f GB), no flush"
                                   % ((2 * nH.numel() * nH.element_size() + 16 * nH.numel()) / 1e9),
-                               multi_gpu="replicas only"),
+                               multi_gpu="sharded by source, one all-reduce of the photon grid" if args.shard else "replicas only"),
                    rt_step_ms=ms / args.steps, march_ms_per_step=ms_march / args.steps,
                    gpu_launches=int(launches), clocks=clk, e2e=e2e, roofline=roof, cpu_baseline=cpu,
                    stats=dict(iterations=int(st.iterations), peak_pool_rays=int(st.peak_pool_rays),

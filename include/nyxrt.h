@@ -141,6 +141,27 @@ int nyxrt_set_sources(nyxrt_ctx *ctx, int64_t n, const double *pos_xyz, const do
  * Errors: ESTATE (fields / sources / workspace missing), EOVERFLOW, ECUDA. */
 int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma_HI, double *d_heat, nyxrt_stats *h_stats, void *cuda_stream);
 
+/* Source sharding across GPUs: Gamma is a sum over sources, so
+ * each of `world` processes, holding a full replica of the fields and the full source list, traces the
+ * catalogue entries rank, rank + world, ... (the catalogue -- dedup, merge, sort -- is computed by every
+ * process, identically), the per-cell photon counts are summed across processes (one all-reduce, done by the
+ * caller, e.g. torch.distributed over NCCL) and nyxrt_finalise turns the sum into rates:
+ *   nyxrt_set_shard(rank, world); nyxrt_trace_photons(d_photons); all-reduce(d_photons); nyxrt_finalise(d_photons, ...)
+ * With a shard set (world > 1), nyxrt_trace / nyxrt_step_host / nyxrt_timestep return ESTATE.
+ * nyxrt_set_shard(0, 1) restores the default.  Errors: EINVAL. */
+int nyxrt_set_shard(nyxrt_ctx *ctx, int32_t rank, int32_t world);
+
+/* nyxrt_trace up to, not including, the division by n_HI V: d_photons (device, [nz][ny][nx] doubles) receives
+ * the photons absorbed per cell per second from this shard's sources.  *h_stats counts this shard's rays;
+ * n_src_* describe the whole catalogue.  Errors: as nyxrt_trace. */
+int nyxrt_trace_photons(nyxrt_ctx *ctx, double *d_photons, nyxrt_stats *h_stats, void *cuda_stream);
+
+/* Gamma_HI and heating (may be NULL) from a dense photon grid (device pointers), as nyxrt_trace's last stage;
+ * *h_absorbed (host, may be NULL) = sum of d_photons.  Needs the fields of the trace still registered.
+ * Synchronises `stream`.  Errors: EINVAL, ESTATE, ECUDA. */
+int nyxrt_finalise(nyxrt_ctx *ctx, const double *d_photons, double *d_gamma_HI, double *d_heat, double *h_absorbed,
+                   void *cuda_stream);
+
 /* The (deduplicated, merged, sorted) catalogue the last nyxrt_trace used: host
  * pointers with room for `cap` entries; cell_ijk is [cap][3]; radius is the bubble radius in cells
  * (0 when merging was off).  Any of the three arrays may be NULL.  *n_out = catalogue length even

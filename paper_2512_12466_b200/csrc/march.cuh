@@ -79,12 +79,13 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
 
 // ---------------------------------------------------------------------------------------------------
 // Emit (PAPER.md:111, 203 spawn_rays): 12 level-0 rays per catalogue source, L/12 each.
-__global__ void emit_kernel(const LoopState *ls, RayPool pool, const double *cat_L) {
+// Source sharding: shard `rank` of `world` emits the catalogue sources rank, rank + world, ...
+__global__ void emit_kernel(const LoopState *ls, RayPool pool, const double *cat_L, int rank, int world) {
     const long long n = ls->emit_n * 12;
     const long long src0 = ls->emit_src, slot0 = ls->emit_slot;
     for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < n;
          r += (long long)gridDim.x * blockDim.x) {
-        const long long a = src0 + r / 12;
+        const long long a = (src0 + r / 12) * world + rank;
         const uint32_t pix = (uint32_t)(r % 12);
         pool.key[slot0 + r] = ray_key((uint32_t)a, 0, pix);
         pool.s[slot0 + r] = 0.0;
@@ -606,7 +607,8 @@ __global__ void sum_partials_kernel(const double *partial, int n, double *out) {
 // absorber, writes the caller's dense [nz][ny][nx] outputs.
 __global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__ heat, const double *__restrict__ acc,
                                 const double *__restrict__ absorber, int nx, int ny, int nz, double V,
-                                double e_excess, int periodic, double *__restrict__ partial) {
+                                double e_excess, int periodic, double *__restrict__ photons_out,
+                                double *__restrict__ partial) {
     __shared__ double sh[256];
     double sum = 0.0;
     const long long ncell = (long long)nx * ny * nz, px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2);
@@ -625,6 +627,37 @@ __global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__
             if (k == 0) ph += acc[q + nz * pxy];
             if (k == nz - 1) ph += acc[q - nz * pxy];
         }
+        sum += ph;
+        if (photons_out) { photons_out[t] = ph; continue; }     // shard mode: raw photon counts, reduced across GPUs first
+        double g = 0.0, h = 0.0;
+        if (ph != 0.0) {
+            g = ph / (fabs(absorber[q]) * V);
+            h = e_excess * ph / V;
+        }
+        gamma[t] = g;
+        if (heat) heat[t] = h;
+    }
+    sh[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = blockDim.x >> 1; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
+// Finalise from a dense [nz][ny][nx] photon grid (the all-reduced sum of the shards' grids)
+__global__ void finalise_dense_kernel(double *__restrict__ gamma, double *__restrict__ heat,
+                                      const double *__restrict__ photons, const double *__restrict__ absorber, int nx,
+                                      int ny, int nz, double V, double e_excess, double *__restrict__ partial) {
+    __shared__ double sh[256];
+    double sum = 0.0;
+    const long long ncell = (long long)nx * ny * nz, px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2);
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < ncell;
+         t += (long long)gridDim.x * blockDim.x) {
+        const long long i = t % nx, j = (t / nx) % ny, k = t / ((long long)nx * ny);
+        const long long q = (k + 1) * pxy + (j + 1) * px + (i + 1);
+        const double ph = photons[t];
         sum += ph;
         double g = 0.0, h = 0.0;
         if (ph != 0.0) {

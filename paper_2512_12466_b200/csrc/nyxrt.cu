@@ -69,6 +69,7 @@ struct nyxrt_ctx {
     long long n_src, n_dedup, n_cat;
     unsigned long long n_aux_launches;     // own kernels launched outside the ray loop in this trace
     int cat_sel;                           // which of sb.cell[]/L2[]/r[] holds the final catalogue
+    int shard_rank, shard_world;           // source sharding (nyxrt_set_shard); 0 of 1 = everything
     double r2_split[MAXLEV], K[MAXLEV];
     cudaEvent_t ev[4];
     cudaEvent_t tev[4];                    // timestep phases
@@ -340,6 +341,8 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     ctx->g = g;
     ctx->p = p;
     ctx->ncell = (long long)g.nx * g.ny * g.nz;
+    ctx->shard_rank = 0;
+    ctx->shard_world = 1;
     ctx->pcell = (long long)(g.nx + 2) * (g.ny + 2) * (g.nz + 2);
     ctx->idx64 = ctx->pcell >= (1ll << 31);
     const double PI = 0x1.921fb54442d18p+1;
@@ -481,9 +484,9 @@ int nyxrt_set_sources(nyxrt_ctx *ctx, int64_t n, const double *pos, const double
     return NYXRT_OK;
 }
 
-int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs, void *cuda_stream) {
+static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_photons, nyxrt_stats *hs, void *cuda_stream) {
     if (!ctx) return NYXRT_EINVAL;
-    if (!d_gamma) return fail(ctx, NYXRT_EINVAL, "trace: null output");
+    if (!d_gamma && !d_photons) return fail(ctx, NYXRT_EINVAL, "trace: null output");
     if (!ctx->ws || !ctx->have_fields || !ctx->have_sources)
         return fail(ctx, NYXRT_ESTATE, "trace: workspace, fields and sources must be set first");
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -501,13 +504,15 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     if (rc) return rc;
     ctx->have_catalog = true;
     const SrcBufs &s = ctx->sb;
-    sum_flux_kernel<<<1, 256, 0, st>>>(s.L2[0], ctx->n_cat, ctx->scalars + 2);
+    sum_flux_kernel<<<1, 256, 0, st>>>(s.L2[0], ctx->n_cat, ctx->shard_rank, ctx->shard_world, ctx->scalars + 2);
+    // this shard's sources: catalogue entries rank, rank + world, ... (all of them when world = 1)
+    const long long n_local = ctx->n_cat > ctx->shard_rank ? (ctx->n_cat - ctx->shard_rank + ctx->shard_world - 1) / ctx->shard_world : 0;
     CU(cudaEventRecord(ctx->ev[1], st));
     // ---- ray loop ----
     CU(cudaMemsetAsync(ctx->acc, 0, ctx->pcell * sizeof(double), st));
     CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
     memset(ctx->h_ls, 0, sizeof(LoopState));
-    ctx->h_ls->n_cat = ctx->n_cat;
+    ctx->h_ls->n_cat = n_local;
     ctx->h_ls->batch_rays = ctx->batch_rays;
     ctx->h_ls->tune_seg_round = ctx->tune_seg_round;
     CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
@@ -536,7 +541,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     for (;;) {
         for (int i = 0; i < chunk; ++i) {
             sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev);
-            emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0]);
+            emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0], ctx->shard_rank, ctx->shard_world);
             if (n_launch + 1 > ctx->mev_cap / 2) {                       // grow the event pool
                 const long long cap = ctx->mev_cap ? 2 * ctx->mev_cap : 1024;
                 cudaEvent_t *m = (cudaEvent_t *)realloc(ctx->mev, cap * sizeof(cudaEvent_t));
@@ -565,7 +570,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     // ---- finalise ----
     const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
     finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->acc, ctx->absorber, ctx->g.nx, ctx->g.ny, ctx->g.nz, V,
-                                              ctx->p.e_excess_erg, ctx->g.periodic, ctx->partial);
+                                              ctx->p.e_excess_erg, ctx->g.periodic, d_photons, ctx->partial);
     sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
     CU(cudaEventRecord(ctx->ev[3], st));
     CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));
@@ -586,7 +591,7 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
         hs->n_src_merged = (uint64_t)ctx->n_cat;
         hs->iterations = ctx->h_ls->iterations;
         hs->peak_pool_rays = ctx->h_ls->peak_pool;
-        hs->photons_emitted = ctx->n_cat ? ctx->h_scalars[2] : 0.0;
+        hs->photons_emitted = n_local ? ctx->h_scalars[2] : 0.0;
         hs->photons_absorbed = ctx->h_scalars[1];
         hs->photons_escaped = d.escaped;
         hs->photons_residual = d.residual;
@@ -606,6 +611,45 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
         hs->march_launches = (uint64_t)live;
         hs->kernel_launches = (uint64_t)(3 * n_launch) + ctx->n_aux_launches;
     }
+    return NYXRT_OK;
+}
+
+int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs, void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!d_gamma) return fail(ctx, NYXRT_EINVAL, "trace: null output");
+    if (ctx->shard_world != 1) return fail(ctx, NYXRT_ESTATE, "trace: a shard is set; use trace_photons + finalise");
+    return run_trace(ctx, d_gamma, d_heat, nullptr, hs, cuda_stream);
+}
+
+int nyxrt_set_shard(nyxrt_ctx *ctx, int32_t rank, int32_t world) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (world < 1 || rank < 0 || rank >= world) return fail(ctx, NYXRT_EINVAL, "set_shard: need 0 <= rank < world");
+    ctx->shard_rank = rank;
+    ctx->shard_world = world;
+    return NYXRT_OK;
+}
+
+int nyxrt_trace_photons(nyxrt_ctx *ctx, double *d_photons, nyxrt_stats *hs, void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!d_photons) return fail(ctx, NYXRT_EINVAL, "trace_photons: null output");
+    return run_trace(ctx, nullptr, nullptr, d_photons, hs, cuda_stream);
+}
+
+int nyxrt_finalise(nyxrt_ctx *ctx, const double *d_photons, double *d_gamma, double *d_heat, double *h_absorbed,
+                   void *cuda_stream) {
+    if (!ctx) return NYXRT_EINVAL;
+    if (!d_photons || !d_gamma) return fail(ctx, NYXRT_EINVAL, "finalise: null pointer");
+    if (!ctx->ws || !ctx->have_fields) return fail(ctx, NYXRT_ESTATE, "finalise: workspace and fields must be set first");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaSetDevice(ctx->g.device));
+    const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
+    finalise_dense_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, d_photons, ctx->absorber, ctx->g.nx, ctx->g.ny,
+                                                    ctx->g.nz, V, ctx->p.e_excess_erg, ctx->partial);
+    sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
+    CU(cudaMemcpyAsync(ctx->h_scalars + 1, ctx->scalars + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    CU(cudaGetLastError());
+    if (h_absorbed) *h_absorbed = ctx->h_scalars[1];
     return NYXRT_OK;
 }
 

@@ -297,10 +297,10 @@ __global__ void fill_double_kernel(double *p, long long n, double v) {
 }
 
 // sum of catalogue fluxes = photons emitted (fixed order: single block, strided then tree)
-__global__ void sum_flux_kernel(const double *__restrict__ L, long long n, double *out) {
+__global__ void sum_flux_kernel(const double *__restrict__ L, long long n, long long first, long long stride, double *out) {
     __shared__ double sh[256];
     double acc = 0.0;
-    for (long long i = threadIdx.x; i < n; i += blockDim.x) acc += L[i];
+    for (long long i = first + (long long)threadIdx.x * stride; i < n; i += (long long)blockDim.x * stride) acc += L[i];
     sh[threadIdx.x] = acc;
     __syncthreads();
     for (int o = blockDim.x >> 1; o > 0; o >>= 1) {

@@ -73,7 +73,8 @@ class nyxrt_tstats(C.Structure):
 EXPORTS = ["nyxrt_create", "nyxrt_workspace_bytes", "nyxrt_set_workspace", "nyxrt_set_fields", "nyxrt_set_sources",
            "nyxrt_trace", "nyxrt_get_catalog", "nyxrt_step_host", "nyxrt_pix2dir", "nyxrt_last_error",
            "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats",
-           "nyxrt_timestep", "nyxrt_sizeof_ode", "nyxrt_sizeof_tstats"]
+           "nyxrt_timestep", "nyxrt_sizeof_ode", "nyxrt_sizeof_tstats", "nyxrt_set_shard", "nyxrt_trace_photons",
+           "nyxrt_finalise"]
 
 _lib = None
 
@@ -159,6 +160,28 @@ def nyxrt_trace(ctx, gamma, heat=None, stream=None):
                                   C.c_void_p(heat.data_ptr()) if heat is not None else None,
                                   C.byref(st), _stream_ptr(stream)))
     return st
+
+
+def nyxrt_set_shard(ctx, rank, world):
+    _check(ctx, lib().nyxrt_set_shard(ctx, C.c_int32(rank), C.c_int32(world)))
+
+
+def nyxrt_trace_photons(ctx, photons, stream=None):
+    assert photons.is_cuda and photons.dtype == torch.float64 and photons.is_contiguous()
+    st = nyxrt_stats()
+    _check(ctx, lib().nyxrt_trace_photons(ctx, C.c_void_p(photons.data_ptr()), C.byref(st), _stream_ptr(stream)))
+    return st
+
+
+def nyxrt_finalise(ctx, photons, gamma, heat=None, stream=None):
+    """Returns the sum of `photons` (absorbed photons per second)."""
+    for t in (photons, gamma) + ((heat,) if heat is not None else ()):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    absorbed = C.c_double(0.0)
+    _check(ctx, lib().nyxrt_finalise(ctx, C.c_void_p(photons.data_ptr()), C.c_void_p(gamma.data_ptr()),
+                                     C.c_void_p(heat.data_ptr()) if heat is not None else None, C.byref(absorbed),
+                                     _stream_ptr(stream)))
+    return absorbed.value
 
 
 def nyxrt_timestep(ctx, ode, nH, xHI_begin, xHI_end, xHI_avg, gamma, heat=None, stream=None):
@@ -288,6 +311,30 @@ class Tracer:
         self._fields = (nH, xa)
         st, ts = nyxrt_timestep(self.ctx, ode, nH, xHI_begin, xe, xa, gamma, heat, stream)
         return xe, xa, gamma, heat, st, ts
+
+    def set_shard(self, rank, world):
+        nyxrt_set_shard(self.ctx, rank, world)
+
+    def trace_photons(self, photons=None, stream=None):
+        if photons is None:
+            photons = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        return photons, nyxrt_trace_photons(self.ctx, photons, stream)
+
+    def finalise(self, photons, want_heat=True, stream=None):
+        gamma = torch.empty(self.shape, dtype=torch.float64, device=self.device)
+        heat = torch.empty(self.shape, dtype=torch.float64, device=self.device) if want_heat else None
+        absorbed = nyxrt_finalise(self.ctx, photons, gamma, heat, stream)
+        return gamma, heat, absorbed
+
+    def sharded_trace(self, group=None, want_heat=True, stream=None):
+        """One RT step sharded by source over the ranks of a torch.distributed group (NCCL): this rank's shard
+        must have been set with set_shard(rank, world).  One all-reduce of the per-cell photon counts."""
+        import torch.distributed as dist
+        photons, st = self.trace_photons(stream=stream)
+        if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+            dist.all_reduce(photons, op=dist.ReduceOp.SUM, group=group)
+        gamma, heat, absorbed = self.finalise(photons, want_heat, stream)
+        return gamma, heat, st, absorbed
 
     def catalog(self):
         return nyxrt_get_catalog(self.ctx)

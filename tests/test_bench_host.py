@@ -18,7 +18,7 @@ def _worker(rank, world, port, out):
     import bench
     dist.init_process_group("gloo", rank=rank, world_size=world)
     ms = bench.max_over_ranks(100.0 + 50.0 * rank, "cpu")        # rank 1 is the slow one
-    out[rank] = (ms, bench.whole_job_rate(1000, ms, world))
+    out[rank] = (ms, bench.whole_job_rate(1000, ms, world), bench.sum_over_ranks(700 + 300 * rank, "cpu"))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -30,8 +30,9 @@ def test_replicas_rate_is_all_units_over_slowest_rank():
         mp.spawn(_worker, args=(world, 29533, out), nprocs=world, join=True)
         res = dict(out)
     assert res[0] == res[1]
-    ms, rate = res[0]
+    ms, rate, seg_all = res[0]
     assert ms == 150.0 and abs(rate - 2 * 1000 / 0.150) < 1e-9
+    assert seg_all == 1700.0                                      # sharded mode: the ranks' own segments add up
 
 
 def test_single_process_identity():
@@ -39,6 +40,7 @@ def test_single_process_identity():
     import bench
     assert bench.max_over_ranks(12.5, "cpu") == 12.5
     assert bench.whole_job_rate(10, 1000.0, 1) == 10.0
+    assert bench.sum_over_ranks(3.0, "cpu") == 3.0
 
 
 def test_reference_arm_other_ranks_exit_quietly():
