@@ -30,11 +30,11 @@ def cfg5():
     return synth.make(5, device="cuda")
 
 
-def _trace(cfg, pos, L, params=None, batch_rays=0):
+def _trace(cfg, pos, L, params=None, batch_rays=0, periodic=0):
     p = dict(cfg["params"])
     p.update(params or {})
     tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], p, field_dtype=cfg["nH"].dtype, max_sources=max(len(L), 1),
-                      batch_rays=batch_rays)
+                      batch_rays=batch_rays, periodic=periodic)
     try:
         tr.set_fields(cfg["nH"], cfg["xHI"])
         tr.set_sources(pos, L)
@@ -123,11 +123,13 @@ def test_configs_3_4_full_grid_sampled_sources(O, config_id, n_sample):
           % (config_id, n_sample, sg.segments, worst))
 
 
-def test_64bit_cell_index_path(O):
+@pytest.mark.parametrize("periodic", [0, 1])
+def test_64bit_cell_index_path(O, periodic):
     """Maximum size: a padded grid of more than 2^31 cells switches the march to 64-bit cell indices
     (march_kernel<GEOM, long long>).  Non-cubic 1026 x 1022 x 2046 fp32 grid, moderately thick medium so that
     the oracle finishes in seconds, sources at both ends of the index range (the last one in the far corner,
-    linear index > 2^31) and next to three faces."""
+    linear index > 2^31) and next to three faces.  periodic = 1: the same box with wrap-around (the corner
+    sources light the opposite corners through the faces; march_kernel<GEOM, long long, true>)."""
     if torch.cuda.mem_get_info()[1] < 150e9:
         pytest.skip("needs the B200's memory")
     nz, ny, nx = 1026, 1022, 2046
@@ -140,13 +142,16 @@ def test_64bit_cell_index_path(O):
                                      [2045.9, 1021.9, 1025.9]], dtype=torch.float64),
                src_L=torch.tensor([1e50, 3e50, 2e49, 5e50], dtype=torch.float64),
                params=synth.default_params(n_th=6e-4, e_excess_erg=1e-11))
-    gam, heat, sg, cg = _trace(cfg, cfg["src_pos"].numpy(), cfg["src_L"].numpy(), batch_rays=2 ** 20)
-    go, ho, so, co = run_oracle(O, cfg)
+    gam, heat, sg, cg = _trace(cfg, cfg["src_pos"].numpy(), cfg["src_L"].numpy(), batch_rays=2 ** 20,
+                             periodic=periodic)
+    go, ho, so, co = run_oracle(O, cfg, periodic=periodic)
     assert np.array_equal(cg[0], co[0]) and np.array_equal(cg[1], co[1])
     for name in COUNTERS:
         assert list(getattr(sg, name)) == list(getattr(so, name)), name
     assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
-    assert sum(sg.exited) > 0 and sum(sg.killed_tau) > 0 and sg.segments > 10 ** 6
+    assert (sum(sg.exited) > 0) == (periodic == 0) and sum(sg.killed_tau) > 0 and sg.segments > 10 ** 6
+    if periodic:
+        assert float(gam[0, 0, 0]) > 0.0 and float(gam[-1, -1, 0]) > 0.0   # lit through the faces
     worst = compare_slabs(gam, heat, go, ho, cfg)
     assert float(gam[-1, -1, -1]) > 0.0                       # the far corner cell (largest index) was lit
     assert_budget(sg, "gpu")
