@@ -400,6 +400,88 @@ int orc_merge(const orc_grid *g, const orc_params *p, int64_t n, const int32_t *
 /* ------------------------------------------------------------------------------------------ */
 /* O3-O7: the ray loop.                                                                          */
 
+/* ------------------------------------------------------------------------------------------ */
+/* S1-S3: frequency-integrated flux (Sec. 2.2): "the solution to Eq. 1 can be      */
+/* precomputed as a function of tau_0 (optical depth at the ionization threshold frequency). A     */
+/* lookup table allows us to sidestep the need for per-ray frequency bins".  With sigma_nu =        */
+/* sigma_0 (nu/nu_0)^-3 (R37) and a photon-number spectrum phi(nu), int phi = 1, the photons a ray  */
+/* of share w loses between tau_0 = a and b are w [Q(b) - Q(a)],                                    */
+/*     Q(tau_0) = int phi(nu) (1 - exp(-tau_0 (nu/nu_0)^-3)) dnu          (Eq. 1's numerator),      */
+/* which telescopes along the ray (photon conservation).  Q is tabulated on nodes fixed by the      */
+/* binary representation of tau_0 (R38): 2^m nodes per octave, linear in tau_0 inside an octave,    */
+/* from 2^e_lo to 2^e_hi; linear from 0 below 2^e_lo; constant above 2^e_hi.                        */
+
+static struct { int on, e_lo, e_hi, m; int64_t n; double *q; } g_lut;
+
+int64_t orc_spectrum_nodes(int e_lo, int e_hi, int m) { return (((int64_t)(e_hi - e_lo)) << m) + 1; }
+
+/* tau_0 of node k */
+double orc_spectrum_node_tau(int e_lo, int m, int64_t k) {
+    int64_t oct = k >> m, sub = k & (((int64_t)1 << m) - 1);
+    return ldexp(1.0 + (double)sub / (double)((int64_t)1 << m), e_lo + (int)oct);
+}
+
+int orc_set_spectrum(int e_lo, int e_hi, int m, const double *q, int64_t n) {
+    free(g_lut.q);
+    memset(&g_lut, 0, sizeof g_lut);
+    if (!q) return ORC_OK;                                              /* back to monochromatic */
+    if (e_lo < -1000 || e_hi > 1000 || e_hi <= e_lo || m < 0 || m > 20 || n != orc_spectrum_nodes(e_lo, e_hi, m))
+        return ORC_EINVAL;
+    g_lut.q = malloc((size_t)n * sizeof *q);
+    if (!g_lut.q) return ORC_ENOMEM;
+    memcpy(g_lut.q, q, (size_t)n * sizeof *q);
+    g_lut.on = 1; g_lut.e_lo = e_lo; g_lut.e_hi = e_hi; g_lut.m = m; g_lut.n = n;
+    return ORC_OK;
+}
+
+/* S2: table lookup (R38) */
+double orc_spectrum_q(double tau) {
+    if (!(tau > 0.0)) return 0.0;
+    if (tau < ldexp(1.0, g_lut.e_lo)) return g_lut.q[0] * ldexp(tau, -g_lut.e_lo);
+    if (tau >= ldexp(1.0, g_lut.e_hi)) return g_lut.q[g_lut.n - 1];
+    uint64_t bits;
+    memcpy(&bits, &tau, sizeof bits);
+    const int fb = 52 - g_lut.m;                                        /* mantissa bits below the node */
+    int64_t k = (int64_t)(bits >> fb) - ((int64_t)(g_lut.e_lo + 1023) << g_lut.m);
+    double frac = ldexp((double)(bits & (((uint64_t)1 << fb) - 1)), -fb);
+    return fma(frac, g_lut.q[k + 1] - g_lut.q[k], g_lut.q[k]);
+}
+
+/* absorbed fraction of a ray's share between the source and optical depth tau; photons absorbed in a
+   segment from tau to tau + dtau (Eq. 1 with V_box) */
+static double remaining_at(double tau) { return g_lut.on ? 1.0 - orc_spectrum_q(tau) : exp(-tau); }
+static double absorbed_in(double tau, double dtau) {
+    if (g_lut.on) return orc_spectrum_q(tau + dtau) - orc_spectrum_q(tau);
+    return exp(-tau) * (-expm1(-dtau));
+}
+
+/* S3: Q of a black body of temperature T_eff [K] (R39): phi(nu) ~ nu^2 / (exp(h nu / k T) - 1) above
+   nu_0 (13.6 eV): with x = h nu / k T, x_0 = h nu_0 / k T,
+       Q(tau) = int_{x0}^inf x^2/(e^x - 1) (1 - exp(-tau (x/x0)^-3)) dx / int_{x0}^inf x^2/(e^x - 1) dx,
+   composite Simpson on u in [0, 1) with x = x0 + u/(1-u) (the integrand vanishes at u -> 1). */
+static double bb_integral(double x0, double tau, int with_abs) {
+    const int N = 20000;                                                /* even */
+    double sum = 0.0;
+    for (int i = 0; i < N; ++i) {                                       /* u = 1 excluded: integrand 0 */
+        double u = (double)i / (double)N;
+        double x = x0 + u / (1.0 - u);
+        double jac = 1.0 / ((1.0 - u) * (1.0 - u));
+        double f = x * x / expm1(x) * jac;
+        if (with_abs) { double r = x0 / x; f *= -expm1(-tau * r * r * r); }
+        double wgt = (i == 0) ? 1.0 : ((i & 1) ? 4.0 : 2.0);
+        sum += wgt * f;
+    }
+    return sum / (3.0 * (double)N);
+}
+
+int orc_blackbody_table(double t_eff_K, int e_lo, int e_hi, int m, double *q, int64_t n) {
+    if (!(t_eff_K > 0.0) || n != orc_spectrum_nodes(e_lo, e_hi, m)) return ORC_EINVAL;
+    const double x0 = 13.598434 * 1.602176634e-19 / (1.380649e-23 * t_eff_K);   /* h nu_0 / k T */
+    const double norm = bb_integral(x0, 0.0, 0);
+    for (int64_t k = 0; k < n; ++k) q[k] = bb_integral(x0, orc_spectrum_node_tau(e_lo, m, k), 1) / norm;
+    return ORC_OK;
+}
+
 typedef struct {
     const orc_grid *g;
     const orc_params *p;
@@ -440,27 +522,27 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
     }
     if (!g->periodic && !in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
         st->exited[level]++;
-        T->escaped += (long double)(L_ray * exp(-tau));
+        T->escaped += (long double)(L_ray * remaining_at(tau));
         return;
     }
     for (;;) {
         /* 1. kill (RAY_FLTR tau test; per cell, R14) */
         if (tau >= p->tau_max) {
             st->killed_tau[level]++;
-            T->residual += (long double)(L_ray * exp(-tau));
+            T->residual += (long double)(L_ray * remaining_at(tau));
             return;
         }
         /* 2. l_max */
         if (level >= p->level_max) {
             st->killed_lmax[level]++;
-            T->residual += (long double)(L_ray * exp(-tau));
+            T->residual += (long double)(L_ray * remaining_at(tau));
             return;
         }
         /* 2b. periodic box: the ray ends once its travel distance is no longer below sqrt(3) L_box
            (RAY_FLTR); counted with the rays that left the system (reading R30) */
         if (g->periodic && !(s < T->s_max)) {
             st->exited[level]++;
-            T->escaped += (long double)(L_ray * exp(-tau));
+            T->escaped += (long double)(L_ray * remaining_at(tau));
             return;
         }
         /* 3. split, Eq. 4: Omega_c/Omega(l) < N_min  <=>  s^2 > 3 4^l/(pi N_min) */
@@ -484,7 +566,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
             double nH_c = fld(T->nH, g->field_dtype, c);
             double a_c = nH_c * fld(T->xHI, g->field_dtype, c);        /* absorber density, PAPER.md:229 (R1) */
             double dtau = (a_c * T->sdx) * ds;                         /* Eq. 2 */
-            double dN = L_ray * exp(-tau) * (-expm1(-dtau));           /* Eq. 1 with V_box */
+            double dN = L_ray * absorbed_in(tau, dtau);                /* Eq. 1 with V_box */
             if (dN > 0.0) {
                 double fc = 1.0, d_edge = 0.0, l_pix = 0.0, a_n = 0.0;
                 int face = -1;
@@ -563,7 +645,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
         sx[ax] = ((double)(o[ax] + (d[ax] > 0.0 ? 1 : 0)) - 0.5) * inv[ax];
         if (!g->periodic && !in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
             st->exited[level]++;                                        /* R20 */
-            T->escaped += (long double)(L_ray * exp(-tau));
+            T->escaped += (long double)(L_ray * remaining_at(tau));
             return;
         }
     }

@@ -272,3 +272,40 @@ def timestep(g, p, o, nH, xHI_begin, pos, L, want_heat=True):
                             C.byref(ts), _ptr(cc), _ptr(cL), _ptr(cr), C.byref(ncat)), "timestep")
     m = ncat.value
     return xe, xa, gamma, heat, st, ts, (cc[:m].copy(), cL[:m].copy(), cr[:m].copy())
+
+
+# ---- frequency-integrated flux: the tau_0 lookup table of PAPER.md:95 -------------------------------------
+
+def spectrum_nodes(e_lo, e_hi, m):
+    f = lib().orc_spectrum_nodes
+    f.restype = C.c_int64
+    return f(C.c_int(e_lo), C.c_int(e_hi), C.c_int(m))
+
+
+def spectrum_node_tau(e_lo, m, k):
+    f = lib().orc_spectrum_node_tau
+    f.restype = C.c_double
+    return f(C.c_int(e_lo), C.c_int(m), C.c_int64(k))
+
+
+def set_spectrum(e_lo=0, e_hi=0, m=0, q=None):
+    """q = None: monochromatic (the default).  The table is copied; it is module state of the oracle."""
+    if q is None:
+        _chk(lib().orc_set_spectrum(0, 0, 0, None, C.c_int64(0)), "set_spectrum")
+        return
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    _chk(lib().orc_set_spectrum(C.c_int(e_lo), C.c_int(e_hi), C.c_int(m), _ptr(q), C.c_int64(len(q))), "set_spectrum")
+
+
+def spectrum_q(tau):
+    f = lib().orc_spectrum_q
+    f.restype = C.c_double
+    return f(C.c_double(tau))
+
+
+def blackbody_table(t_eff_K, e_lo, e_hi, m):
+    n = spectrum_nodes(e_lo, e_hi, m)
+    q = np.zeros(n)
+    _chk(lib().orc_blackbody_table(C.c_double(t_eff_K), C.c_int(e_lo), C.c_int(e_hi), C.c_int(m), _ptr(q), C.c_int64(n)),
+         "blackbody_table")
+    return q
