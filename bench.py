@@ -36,6 +36,9 @@ def parse():
     ap.add_argument("--batch-rays", type=int, default=0)
     ap.add_argument("--shard", action="store_true",
                     help="N > 1: shard the step by source (one all-reduce of the photon grid) instead of N replicas")
+    ap.add_argument("--spectrum-teff", type=float, default=0.0,
+                    help="trace with the tau_0 lookup table of a black body of this temperature [K] (default: monochromatic)")
+    ap.add_argument("--periodic", action="store_true", help="periodic box (default: BASELINE.json's open box)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -212,7 +215,10 @@ def main():
     nH, xHI = cfg["nH"], cfg["xHI"]
     fdt = "f32" if nH.dtype == torch.float32 else "f64"
     tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], cfg["params"], field_dtype=nH.dtype, max_sources=len(L),
-                      batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local)
+                      batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local,
+                      periodic=1 if args.periodic else 0)
+    if args.spectrum_teff > 0:
+        tr.set_spectrum(-20, 12, 8, nyxrt.nyxrt_blackbody_table(args.spectrum_teff, -20, 12, 8))
     gam = torch.empty(cfg["shape"], dtype=torch.float64, device="cuda")
     heat = torch.empty_like(gam)
     stream = torch.cuda.current_stream()
@@ -317,7 +323,10 @@ def main():
                                segments_per_step=int(seg_all // (args.steps * (1 if args.shard else world))), notes=cfg["notes"],
                                l2="inputs larger than L2 (fields + accumulator = %.1f GB), no flush"
                                   % ((2 * nH.numel() * nH.element_size() + 16 * nH.numel()) / 1e9),
-                               multi_gpu="sharded by source, one all-reduce of the photon grid" if args.shard else "replicas only"),
+                               multi_gpu="sharded by source, one all-reduce of the photon grid" if args.shard else "replicas only",
+                               periodic=bool(args.periodic),
+                               spectrum=("black body %g K, tau_0 table 2^-20..2^12, 256 nodes per octave" % args.spectrum_teff)
+                               if args.spectrum_teff > 0 else "monochromatic"),
                    rt_step_ms=ms / args.steps, march_ms_per_step=ms_march / args.steps,
                    gpu_launches=int(launches), clocks=clk, e2e=e2e, roofline=roof, cpu_baseline=cpu,
                    stats=dict(iterations=int(st.iterations), peak_pool_rays=int(st.peak_pool_rays),

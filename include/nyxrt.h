@@ -141,6 +141,26 @@ int nyxrt_set_sources(nyxrt_ctx *ctx, int64_t n, const double *pos_xyz, const do
  * Errors: ESTATE (fields / sources / workspace missing), EOVERFLOW, ECUDA. */
 int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma_HI, double *d_heat, nyxrt_stats *h_stats, void *cuda_stream);
 
+/* Frequency-integrated flux (Sec. 2.2: Eq. 1 "precomputed as a function of tau_0 ... a lookup
+ * table"; cross-section sigma_nu = sigma_cm2 (nu/nu_0)^-3, R37).  The table holds the absorbed fraction
+ *     Q(tau_0) = int phi(nu) (1 - exp(-tau_0 (nu/nu_0)^-3)) dnu,   phi = photon-number spectrum, int phi = 1,
+ * of a ray's share between the source and threshold optical depth tau_0; a segment from tau_0 = a to b absorbs
+ * share * [Q(b) - Q(a)] photons (Eq. 1's numerator; telescopes along the ray).  Nodes are fixed by the binary
+ * representation of tau_0 (R38): node k = 2^(e_lo + (k >> m)) * (1 + (k mod 2^m) / 2^m), k = 0 .. (e_hi - e_lo) 2^m;
+ * Q is linear in tau_0 between nodes, linear from 0 below 2^e_lo, constant above 2^e_hi.
+ *   nyxrt_spectrum_nodes      number of nodes n (m <= 16, n <= 2^24)
+ *   nyxrt_spectrum_node_tau   tau_0 of node k
+ *   nyxrt_set_spectrum        h_q: host array of n values, non-decreasing in [0, 1]; copied to the device
+ *                             (a small cudaMalloc owned by the context).  h_q = NULL: monochromatic again
+ *                             (the default: Q = 1 - e^-tau evaluated in the kernel).  Needs geom_mode 2 or 3.
+ *                             Choose tau_max (nyxrt_params) for the spectrum: hard photons outlive tau_0 = ln 1e8.
+ *   nyxrt_blackbody_table     fills h_q with Q of a black body of temperature t_eff_K above 13.6 eV (R39)
+ * Heating stays e_excess_erg per absorbed photon (H1).  Errors: EINVAL, ECUDA. */
+int nyxrt_spectrum_nodes(int32_t e_lo, int32_t e_hi, int32_t m, int64_t *n);
+int nyxrt_spectrum_node_tau(int32_t e_lo, int32_t m, int64_t k, double *tau);
+int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, const double *h_q, int64_t n);
+int nyxrt_blackbody_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_q, int64_t n);
+
 /* Source sharding across GPUs: Gamma is a sum over sources, so
  * each of `world` processes, holding a full replica of the fields and the full source list, traces the
  * catalogue entries rank, rank + world, ... (the catalogue -- dedup, merge, sort -- is computed by every

@@ -3,7 +3,7 @@
  *
  * A plain, slow, single-threaded fp64 CPU statement of ONE adaptive ray-tracing step on a
  * uniform coarse grid, written from the paper (arxiv 2512.12466, text at
- * /root/reference/PAPER.md; "PAPER.md:<line>" below) with the readings R1..R36 recorded in
+ * /root/reference/PAPER.md; "PAPER.md:<line>" below) with the readings R1..R39 recorded in
  * DESIGN.md ("Readings").  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
  * --impl reference leg may load this file.  It shares no code, header, table or helper with the
  * CUDA library under paper_2512_12466_b200/csrc and neither includes the other.

@@ -150,7 +150,23 @@ enum { OUT_NONE = 0, OUT_SPLIT = 1, OUT_KILL_TAU = 2, OUT_EXIT = 3, OUT_KILL_LMA
 struct ThreadScratch {
     unsigned long long key[MARCH_THREADS];
     double esc[MARCH_THREADS], res[MARCH_THREADS];
+    double w[MARCH_THREADS];             // spectrum table: the ray's share of its source's photons (constant)
 };
+
+// Frequency-integrated flux (Sec. 2.2): absorbed fraction Q(tau_0) of a ray's share between the
+// source and threshold optical depth tau_0, tabulated on the binary buckets of tau_0 (2^m nodes per octave from
+// 2^e_lo to 2^e_hi, linear in tau_0 inside a bucket; linear from 0 below the table, constant above it: R38).
+// Bit operations and one fma: the same number on the host oracle and here.
+__device__ __forceinline__ double lut_q(const MarchArgs &A, double tau) {
+    if (!(tau > 0.0)) return 0.0;
+    if (tau < A.lut_t_lo) return A.lut_q_first * (tau * A.lut_inv_t_lo);
+    if (tau >= A.lut_t_hi) return A.lut_q_last;
+    const long long bits = __double_as_longlong(tau);
+    const long long k = (bits >> A.lut_fb) - A.lut_k0;
+    const double frac = (double)(bits & A.lut_fmask) * A.lut_fscale;
+    const double q0 = __ldg(A.lut_q + k), q1 = __ldg(A.lut_q + k + 1);
+    return fma(frac, q1 - q0, q0);
+}
 
 // One ray-cell segment, described by the geometry stage and consumed by the physics stage one iteration
 // later (so that its two absorber gathers have a whole iteration to arrive).
@@ -185,7 +201,9 @@ constexpr unsigned long long WRAP_MASK = (1ull << WRAP_BITS) - 1ull;
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
 // PER: periodic box: cells wrap, rays end at s >= sqrt(3) L_box, the halo holds the wrapped
 // images of the opposite faces (neighbour reads) and deposits into it are folded back by finalise.
-template <int GEOM, typename IDX, bool PER>
+// LUT: absorbed photons from the spectrum table, w [Q(tau + dtau) - Q(tau)], instead of the monochromatic
+// N (1 - e^-dtau); the lane's N register then holds Q(tau) and the pool's N the share w.
+template <int GEOM, typename IDX, bool PER, bool LUT>
 __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(const __grid_constant__ MarchArgs A) {
     __shared__ ThreadScratch T;
     __shared__ RayQueue<IDX> Q;
@@ -320,9 +338,14 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             if (D.ds > 0.0) {
                 ++n_seg;
                 const double dtau = (fabs(D.a_c) * sdx) * D.ds;
-                double pm, left;
-                absorb_fraction(dtau, pm, left);
-                const double dN = N * (-pm);
+                double pm, left, dN;
+                if (LUT) {
+                    left = lut_q(A, tau + dtau);                                  // Q at the end of the segment
+                    dN = T.w[threadIdx.x] * (left - N);
+                } else {
+                    absorb_fraction(dtau, pm, left);
+                    dN = N * (-pm);
+                }
                 if (dN > 0.0) {
                     double fc = 1.0;
                     if (GEOM == 3) {
@@ -336,7 +359,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                     }
                     atomicAdd(acc + D.c, fc * dN);
                 }
-                N = N * left;
+                N = LUT ? left : N * left;
                 tau = tau + dtau;
             } else {
                 ++n_zero;
@@ -346,7 +369,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     };
 
     // retire rays whose outcome is known (all lanes call it; outcome NONE = nothing to do)
-    auto retire = [&](int outcome, double rs, double rtau, double rN, unsigned long long rkey) {
+    // rN: photons the ray still carries (budget); rW: what its children share (= rN, or the share w with a table)
+    auto retire = [&](int outcome, double rs, double rtau, double rN, double rW, unsigned long long rkey) {
         const unsigned m_any = __ballot_sync(0xffffffffu, outcome != OUT_NONE);
         if (m_any == 0) return;
         const unsigned m_split = __ballot_sync(0xffffffffu, outcome == OUT_SPLIT);
@@ -380,7 +404,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 const long long lo = 4 * __popc(m_split & lt);
                 const long long w = A.pool.off[level + 1] + (lo < rem ? slab_pos + lo : base + (lo - rem));
                 const uint32_t src = key_src(rkey), p4 = 4u * key_pix(rkey);
-                const double Nc = rN * 0.25;                                     // L shared evenly
+                const double Nc = rW * 0.25;                                     // L shared evenly
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     A.pool.key[w + k] = ray_key(src, level + 1, p4 + k);
@@ -462,7 +486,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             qhead = 0;
             qn = __popc(m_park);
             __syncwarp();
-            retire(outcome, ts, ttau, tN, ikey);
+            retire(outcome, ts, ttau, (LUT && outcome != OUT_NONE) ? tN * (1.0 - lut_q(A, ttau)) : tN, tN, ikey);
             continue;
         }
         // ---- pop: idle lanes take parked rays ------------------------------------------------------------
@@ -475,6 +499,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 const int e = qhead + rank;
                 T.key[threadIdx.x] = Q.key[wid][e];
                 s = Q.s[wid][e]; tau = Q.tau[wid][e]; N = Q.N[wid][e];
+                if (LUT) { T.w[threadIdx.x] = N; N = lut_q(A, tau); }
                 d0 = Q.d0[wid][e]; d1 = Q.d1[wid][e]; d2 = Q.d2[wid][e];
                 inv0 = Q.inv0[wid][e]; inv1 = Q.inv1[wid][e]; inv2 = Q.inv2[wid][e];
                 c = Q.c[wid][e];
@@ -517,7 +542,12 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 }
             }
         }
-        retire(outcome, s, tau, N, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
+        if (LUT) {
+            const double w = T.w[threadIdx.x];
+            retire(outcome, s, tau, w * (1.0 - N), w, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
+        } else {
+            retire(outcome, s, tau, N, N, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
+        }
         if (outcome != OUT_NONE) has = false;
     }
     // pad the unused tail of the last child slab

@@ -71,6 +71,10 @@ struct nyxrt_ctx {
     int cat_sel;                           // which of sb.cell[]/L2[]/r[] holds the final catalogue
     int shard_rank, shard_world;           // source sharding (nyxrt_set_shard); 0 of 1 = everything
     double r2_split[MAXLEV], K[MAXLEV];
+    double *d_lut;                         // spectrum table on the device (nyxrt_set_spectrum), or null
+    int lut_e_lo, lut_e_hi, lut_m;
+    long long lut_n;
+    double lut_first, lut_last;
     cudaEvent_t ev[4];
     cudaEvent_t tev[4];                    // timestep phases
     cudaEvent_t *mev;                      // pairs of events around every march launch
@@ -203,14 +207,14 @@ long long default_batch(const nyxrt_ctx *c) {
 
 constexpr size_t MARCH_SMEM = 0;          // the kernel's scratch is static shared memory
 
-template <int GEOM>
+template <int GEOM, bool LUT>
 void launch_march(const MarchArgs &a, bool idx64, bool per, int blocks, cudaStream_t st) {
     if (per) {
-        if (idx64) march_kernel<GEOM, long long, true><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
-        else march_kernel<GEOM, int, true><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+        if (idx64) march_kernel<GEOM, long long, true, LUT><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+        else march_kernel<GEOM, int, true, LUT><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
     } else {
-        if (idx64) march_kernel<GEOM, long long, false><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
-        else march_kernel<GEOM, int, false><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+        if (idx64) march_kernel<GEOM, long long, false, LUT><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
+        else march_kernel<GEOM, int, false, LUT><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
     }
 }
 
@@ -221,10 +225,25 @@ cudaError_t setup_kernel(K kern, int *occ) {
     return e;
 }
 
-template <int GEOM>
+template <int GEOM, bool LUT>
 cudaError_t setup_march(bool idx64, bool per, int *occ) {
-    if (per) return idx64 ? setup_kernel(march_kernel<GEOM, long long, true>, occ) : setup_kernel(march_kernel<GEOM, int, true>, occ);
-    return idx64 ? setup_kernel(march_kernel<GEOM, long long, false>, occ) : setup_kernel(march_kernel<GEOM, int, false>, occ);
+    if (per) return idx64 ? setup_kernel(march_kernel<GEOM, long long, true, LUT>, occ) : setup_kernel(march_kernel<GEOM, int, true, LUT>, occ);
+    return idx64 ? setup_kernel(march_kernel<GEOM, long long, false, LUT>, occ) : setup_kernel(march_kernel<GEOM, int, false, LUT>, occ);
+}
+
+// Q(tau_0) of a black body above the H I threshold (PAPER.md:85-95 with sigma ~ nu^-3, R37/R39), by composite
+// Simpson in v = nu_0 / nu on (0, 1]:  int_{x0}^inf B(x) (1 - exp(-tau (x0/x)^3)) dx,  B = x^2 / (e^x - 1), x = x0 / v.
+double bb_absorbed(double x0, double tau, bool with_abs) {
+    const int N = 40000;
+    double sum = 0.0;
+    for (int i = 1; i <= N; ++i) {                                          // v = 0: the integrand vanishes
+        const double v = (double)i / (double)N;
+        const double x = x0 / v;
+        double f = x * x * std::exp(-x) / -std::expm1(-x) * (x0 / (v * v));
+        if (with_abs) f *= -std::expm1(-tau * v * v * v);
+        sum += (i == N ? 1.0 : ((i & 1) ? 4.0 : 2.0)) * f;
+    }
+    return sum / (3.0 * (double)N);
 }
 
 int geom_template(int mode) { return mode == 2 ? 3 : mode; }
@@ -363,10 +382,16 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     int occ = 0;
     if (e == cudaSuccess) {
         switch (geom_template(p.geom_mode)) {
-            case 0: e = setup_march<0>(ctx->idx64, g.periodic != 0, &occ); break;
-            case 1: e = setup_march<1>(ctx->idx64, g.periodic != 0, &occ); break;
-            case 4: e = setup_march<4>(ctx->idx64, g.periodic != 0, &occ); break;
-            default: e = setup_march<3>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 0: e = setup_march<0, false>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 1: e = setup_march<1, false>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 4: e = setup_march<4, false>(ctx->idx64, g.periodic != 0, &occ); break;
+            default: {
+                int occ_lut = 0;
+                e = setup_march<3, true>(ctx->idx64, g.periodic != 0, &occ_lut);
+                if (e == cudaSuccess) e = setup_march<3, false>(ctx->idx64, g.periodic != 0, &occ);
+                if (occ_lut < occ) occ = occ_lut;
+                break;
+            }
         }
     }
     if (e != cudaSuccess) {
@@ -389,6 +414,7 @@ void nyxrt_destroy(nyxrt_ctx *ctx) {
         if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
     for (int k = 0; k < 4; ++k)
         if (ctx->tev[k]) cudaEventDestroy(ctx->tev[k]);
+    if (ctx->d_lut) cudaFree(ctx->d_lut);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->h_ls) cudaFreeHost(ctx->h_ls);
     if (ctx->h_ds) cudaFreeHost(ctx->h_ds);
@@ -534,6 +560,19 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     a.s_max = std::sqrt((double)((long long)ctx->g.nx * ctx->g.nx + (long long)ctx->g.ny * ctx->g.ny +
                                  (long long)ctx->g.nz * ctx->g.nz));       // sqrt(3) L_box for a cube
     for (int l = 0; l < MAXLEV; ++l) { a.r2_split[l] = ctx->r2_split[l]; a.K[l] = ctx->K[l]; }
+    const bool lut = ctx->d_lut != nullptr;
+    if (lut) {
+        a.lut_q = ctx->d_lut;
+        a.lut_t_lo = std::ldexp(1.0, ctx->lut_e_lo);
+        a.lut_t_hi = std::ldexp(1.0, ctx->lut_e_hi);
+        a.lut_inv_t_lo = std::ldexp(1.0, -ctx->lut_e_lo);
+        a.lut_q_first = ctx->lut_first;
+        a.lut_q_last = ctx->lut_last;
+        a.lut_fb = 52 - ctx->lut_m;
+        a.lut_fscale = std::ldexp(1.0, -a.lut_fb);
+        a.lut_fmask = (1ll << a.lut_fb) - 1;
+        a.lut_k0 = (long long)(ctx->lut_e_lo + 1023) << ctx->lut_m;
+    }
     const int gt = geom_template(ctx->p.geom_mode);
     const int emit_blocks = ctx->sm_count * 4;
     int chunk = 8;
@@ -552,10 +591,13 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
             switch (gt) {
-                case 0: launch_march<0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
-                case 1: launch_march<1>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
-                case 4: launch_march<4>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
-                default: launch_march<3>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 0: launch_march<0, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 1: launch_march<1, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 4: launch_march<4, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                default:
+                    if (lut) launch_march<3, true>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
+                    else launch_march<3, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
+                    break;
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch + 1], st));
             ++n_launch;
@@ -619,6 +661,60 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, nyxrt_stats *hs
     if (!d_gamma) return fail(ctx, NYXRT_EINVAL, "trace: null output");
     if (ctx->shard_world != 1) return fail(ctx, NYXRT_ESTATE, "trace: a shard is set; use trace_photons + finalise");
     return run_trace(ctx, d_gamma, d_heat, nullptr, hs, cuda_stream);
+}
+
+int nyxrt_spectrum_nodes(int32_t e_lo, int32_t e_hi, int32_t m, int64_t *n) {
+    if (!n || e_lo < -1000 || e_hi > 1000 || e_hi <= e_lo || m < 0 || m > 16) return NYXRT_EINVAL;
+    *n = (((int64_t)(e_hi - e_lo)) << m) + 1;
+    return *n <= (1ll << 24) ? NYXRT_OK : NYXRT_EINVAL;
+}
+
+int nyxrt_spectrum_node_tau(int32_t e_lo, int32_t m, int64_t k, double *tau) {
+    if (!tau || m < 0 || m > 16 || k < 0) return NYXRT_EINVAL;
+    const int64_t oct = k >> m, sub = k & (((int64_t)1 << m) - 1);
+    *tau = std::ldexp(1.0 + (double)sub / (double)((int64_t)1 << m), e_lo + (int)oct);
+    return NYXRT_OK;
+}
+
+int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, const double *h_q, int64_t n) {
+    if (!ctx) return NYXRT_EINVAL;
+    CU(cudaSetDevice(ctx->g.device));
+    if (!h_q) {                                                            // back to monochromatic
+        if (ctx->d_lut) cudaFree(ctx->d_lut);
+        ctx->d_lut = nullptr;
+        return NYXRT_OK;
+    }
+    int64_t need = 0;
+    if (nyxrt_spectrum_nodes(e_lo, e_hi, m, &need) != NYXRT_OK || n != need)
+        return fail(ctx, NYXRT_EINVAL, "set_spectrum: bad table geometry or length");
+    if (geom_template(ctx->p.geom_mode) != 3)
+        return fail(ctx, NYXRT_EINVAL, "set_spectrum: the spectrum table needs geom_mode 2 or 3");
+    for (int64_t k = 0; k < n; ++k)
+        if (!(h_q[k] >= 0.0) || !(h_q[k] <= 1.0) || (k > 0 && h_q[k] < h_q[k - 1]))
+            return fail(ctx, NYXRT_EINVAL, "set_spectrum: Q must be non-decreasing within [0, 1]");
+    if (ctx->d_lut) cudaFree(ctx->d_lut);
+    ctx->d_lut = nullptr;
+    CU(cudaMalloc(&ctx->d_lut, n * sizeof(double)));
+    CU(cudaMemcpy(ctx->d_lut, h_q, n * sizeof(double), cudaMemcpyHostToDevice));
+    ctx->lut_e_lo = e_lo; ctx->lut_e_hi = e_hi; ctx->lut_m = m; ctx->lut_n = n;
+    ctx->lut_first = h_q[0];
+    ctx->lut_last = h_q[n - 1];
+    return NYXRT_OK;
+}
+
+int nyxrt_blackbody_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_q, int64_t n) {
+    int64_t need = 0;
+    if (!h_q || !(t_eff_K > 0.0) || nyxrt_spectrum_nodes(e_lo, e_hi, m, &need) != NYXRT_OK || n != need) return NYXRT_EINVAL;
+    const double x0 = 13.598434 * 1.602176634e-19 / (1.380649e-23 * t_eff_K);   // h nu_0 / k T_eff
+    const double norm = bb_absorbed(x0, 0.0, false);
+    for (int64_t k = 0; k < n; ++k) {
+        double tau = 0.0;
+        nyxrt_spectrum_node_tau(e_lo, m, k, &tau);
+        const double q = bb_absorbed(x0, tau, true) / norm;
+        h_q[k] = q > 1.0 ? 1.0 : q;
+        if (k > 0 && h_q[k] < h_q[k - 1]) h_q[k] = h_q[k - 1];              // quadrature noise near Q = 1
+    }
+    return NYXRT_OK;
 }
 
 int nyxrt_set_shard(nyxrt_ctx *ctx, int32_t rank, int32_t world) {

@@ -66,6 +66,11 @@ struct MarchArgs {
     double tau_max;
     double s_max;                        // periodic box: a ray ends once its travel distance s >= sqrt(nx^2+ny^2+nz^2)
                                          // cells = sqrt(3) L_box for a cube
+    // spectrum table, used by the LUT instantiations only
+    const double *lut_q;                 // Q at the nodes
+    double lut_t_lo, lut_t_hi, lut_inv_t_lo, lut_q_first, lut_q_last, lut_fscale;
+    long long lut_k0, lut_fmask;
+    int lut_fb;
     double r2_split[MAXLEV];             // Eq. 4: split when s^2 > 3 4^l / (pi N_min)
     double K[MAXLEV];                    // sqrt(Omega(l)) = sqrt(pi/3) 2^-l: L_pix = R K
 };

@@ -74,7 +74,8 @@ EXPORTS = ["nyxrt_create", "nyxrt_workspace_bytes", "nyxrt_set_workspace", "nyxr
            "nyxrt_trace", "nyxrt_get_catalog", "nyxrt_step_host", "nyxrt_pix2dir", "nyxrt_last_error",
            "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats",
            "nyxrt_timestep", "nyxrt_sizeof_ode", "nyxrt_sizeof_tstats", "nyxrt_set_shard", "nyxrt_trace_photons",
-           "nyxrt_finalise"]
+           "nyxrt_finalise", "nyxrt_spectrum_nodes", "nyxrt_spectrum_node_tau", "nyxrt_set_spectrum",
+           "nyxrt_blackbody_table"]
 
 _lib = None
 
@@ -160,6 +161,42 @@ def nyxrt_trace(ctx, gamma, heat=None, stream=None):
                                   C.c_void_p(heat.data_ptr()) if heat is not None else None,
                                   C.byref(st), _stream_ptr(stream)))
     return st
+
+
+def nyxrt_spectrum_nodes(e_lo, e_hi, m):
+    n = C.c_int64(0)
+    rc = lib().nyxrt_spectrum_nodes(C.c_int32(e_lo), C.c_int32(e_hi), C.c_int32(m), C.byref(n))
+    if rc != OK:
+        raise NyxrtError(rc, "bad table geometry")
+    return n.value
+
+
+def nyxrt_spectrum_node_tau(e_lo, m, k):
+    t = C.c_double(0.0)
+    rc = lib().nyxrt_spectrum_node_tau(C.c_int32(e_lo), C.c_int32(m), C.c_int64(k), C.byref(t))
+    if rc != OK:
+        raise NyxrtError(rc, "bad node")
+    return t.value
+
+
+def nyxrt_set_spectrum(ctx, e_lo=0, e_hi=0, m=0, q=None):
+    """q: host array of Q at the nodes (None: back to monochromatic)."""
+    if q is None:
+        _check(ctx, lib().nyxrt_set_spectrum(ctx, 0, 0, 0, None, C.c_int64(0)))
+        return
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    _check(ctx, lib().nyxrt_set_spectrum(ctx, C.c_int32(e_lo), C.c_int32(e_hi), C.c_int32(m),
+                                         q.ctypes.data_as(C.c_void_p), C.c_int64(len(q))))
+
+
+def nyxrt_blackbody_table(t_eff_K, e_lo, e_hi, m):
+    n = nyxrt_spectrum_nodes(e_lo, e_hi, m)
+    q = np.zeros(n)
+    rc = lib().nyxrt_blackbody_table(C.c_double(t_eff_K), C.c_int32(e_lo), C.c_int32(e_hi), C.c_int32(m),
+                                     q.ctypes.data_as(C.c_void_p), C.c_int64(n))
+    if rc != OK:
+        raise NyxrtError(rc, "blackbody_table: bad argument")
+    return q
 
 
 def nyxrt_set_shard(ctx, rank, world):
@@ -311,6 +348,9 @@ class Tracer:
         self._fields = (nH, xa)
         st, ts = nyxrt_timestep(self.ctx, ode, nH, xHI_begin, xe, xa, gamma, heat, stream)
         return xe, xa, gamma, heat, st, ts
+
+    def set_spectrum(self, e_lo=0, e_hi=0, m=0, q=None):
+        nyxrt_set_spectrum(self.ctx, e_lo, e_hi, m, q)
 
     def set_shard(self, rank, world):
         nyxrt_set_shard(self.ctx, rank, world)
