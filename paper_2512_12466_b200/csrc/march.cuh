@@ -8,10 +8,13 @@
 // four children are pushed on the stack of level+1.
 //
 // Kernel shape (sm_100a, latency- and issue-bound rather than HBM-bound, see profiles/): persistent warps.
-// A warp claims chunks of rays; whenever enough of its lanes are idle they take new rays straight from the
-// batch (HEALPix direction, start cell), so ray-length tails do not idle lanes, and no shared memory is
-// taken from the L1 that serves the field gathers.  The grids are padded by one halo cell holding -inf: leaving the box is "the absorber I
-// just loaded is -inf", a neighbour outside the box is never eligible, and no cell coordinates are tracked.
+// A warp claims chunks of 32 rays, sets them up at full width and parks them in a shared-memory queue; a
+// lane whose ray ended pops the next one, so ray-length tails do not idle lanes.  Per cell the work is split
+// into a geometry stage (DDA, Eq. 5-8 geometry, the two absorber gathers) that runs TWO cells ahead of the
+// physics stage (absorption, deposits), through three segment descriptors in registers.  The ray's read-only
+// direction and 1/d live in shared memory.  The grids are padded by one halo cell holding -inf: leaving the
+// box is "the absorber I just loaded is -inf", a neighbour outside the box is never eligible, and no cell
+// coordinates are tracked.
 //
 // Everything that steers control flow follows DESIGN.md's DEC list literally; this translation unit is
 // compiled with -fmad=false.
@@ -23,7 +26,9 @@ namespace nyxrt {
 
 constexpr int MARCH_THREADS = 128;
 constexpr int MARCH_WARPS = MARCH_THREADS / 32;
-constexpr int MARCH_MIN_BLOCKS = 4;      // 16 warps per SM at <= 128 registers, no spills (checked with -Xptxas -v)
+constexpr int MARCH_MIN_BLOCKS = 4;      // 16 warps per SM at <= 128 registers, no spills (checked with -Xptxas -v); a fifth
+                                         // block (96 registers, 132 KB of shared memory) measured 6 % slower
+constexpr int MARCH_CARVEOUT = 40;       // preferred shared-memory carve-out [% of 228 KB]: 4 blocks x 21 KB
 
 // ---------------------------------------------------------------------------------------------------
 // Scheduler: one thread decides what the next emit + march launches do.
@@ -72,7 +77,7 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->level = pick;
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
-    ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 2 : (pick < 4 ? 4 : (pick < 6 ? 8 : 16)));
+    ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 3 : 21);
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
@@ -147,10 +152,24 @@ __device__ __forceinline__ double signed_half(double x) {
 enum { OUT_NONE = 0, OUT_SPLIT = 1, OUT_KILL_TAU = 2, OUT_EXIT = 3, OUT_KILL_LMAX = 4 };
 
 // per-thread scratch that is touched only when a ray is born or retires (kept out of registers)
+template <bool ON, typename V, int N>
+struct OptArray { V v[N]; };
+template <typename V, int N>
+struct OptArray<false, V, N> {};          // not needed by this instantiation: takes no shared memory
+
+template <bool LUT>
 struct ThreadScratch {
     unsigned long long key[MARCH_THREADS];
     double esc[MARCH_THREADS], res[MARCH_THREADS];
-    double w[MARCH_THREADS];             // spectrum table: the ray's share of its source's photons (constant)
+    OptArray<LUT, double, MARCH_THREADS> w;   // spectrum table: the ray's share of its source's photons (constant)
+    double d[3][MARCH_THREADS];          // the lane's ray: HEALPix direction and 1/d (read-only while it marches;
+    double inv[3][MARCH_THREADS];        // kept out of the register file so that 5 blocks fit an SM)
+};
+
+// warp-uniform bookkeeping that only the retire path touches
+struct WarpScratch {
+    long long slab_pos[MARCH_WARPS], slab_end[MARCH_WARPS];       // child slots reserved on the stack of level+1
+    unsigned int n_split[MARCH_WARPS], n_ktau[MARCH_WARPS], n_exit[MARCH_WARPS], n_klmax[MARCH_WARPS], n_hole[MARCH_WARPS];
 };
 
 // Frequency-integrated flux (Sec. 2.2): absorbed fraction Q(tau_0) of a ray's share between the
@@ -182,14 +201,14 @@ struct SegDesc {
 // Rays of the current chunk that passed their birth tests, initialised at full warp width and parked until
 // a lane falls idle (one queue of FETCH_CHUNK = 32 entries per warp; positions are never stored).
 static_assert(FETCH_CHUNK == 32, "one chunk = one ray per lane");
-template <typename IDX>
+template <typename IDX, bool PER>
 struct RayQueue {
     unsigned long long key[MARCH_WARPS][32];
     double s[MARCH_WARPS][32], tau[MARCH_WARPS][32], N[MARCH_WARPS][32];
     double d0[MARCH_WARPS][32], d1[MARCH_WARPS][32], d2[MARCH_WARPS][32];           // HEALPix direction
     double inv0[MARCH_WARPS][32], inv1[MARCH_WARPS][32], inv2[MARCH_WARPS][32];     // 1/d (-inf where d = 0)
     IDX c[MARCH_WARPS][32];                                                          // start cell
-    unsigned long long cnt[MARCH_WARPS][32];                                         // periodic box: steps to each face
+    OptArray<PER, unsigned long long, MARCH_WARPS * 32> cnt;                         // periodic box: steps to each face
 };
 
 // Periodic box: the ray's cell index stays inside the box.  cnt packs, 21 bits per
@@ -205,8 +224,9 @@ constexpr unsigned long long WRAP_MASK = (1ull << WRAP_BITS) - 1ull;
 // N (1 - e^-dtau); the lane's N register then holds Q(tau) and the pool's N the share w.
 template <int GEOM, typename IDX, bool PER, bool LUT>
 __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(const __grid_constant__ MarchArgs A) {
-    __shared__ ThreadScratch T;
-    __shared__ RayQueue<IDX> Q;
+    __shared__ ThreadScratch<LUT> T;
+    __shared__ RayQueue<IDX, PER> Q;
+    __shared__ WarpScratch W;
     const int wid = threadIdx.x >> 5;
     const LoopState *ls = A.ls;
     const long long batch = ls->batch;
@@ -227,23 +247,26 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     T.esc[threadIdx.x] = 0.0;
     T.res[threadIdx.x] = 0.0;
     unsigned int n_seg = 0, n_zero = 0;
-    unsigned int n_split = 0, n_ktau = 0, n_exit = 0, n_klmax = 0, n_hole = 0;   // lane 0 holds warp totals
     double lost = 0.0;
+    if (lane == 0) {
+        W.slab_pos[wid] = W.slab_end[wid] = 0;
+        W.n_split[wid] = W.n_ktau[wid] = W.n_exit[wid] = W.n_klmax[wid] = W.n_hole[wid] = 0u;
+    }
+    __syncwarp();
 
     // warp-uniform bookkeeping
     int qhead = 0, qn = 0;                          // the warp's parked rays: entries [qhead, qhead+qn)
     bool exhausted = false;
-    long long slab_pos = 0, slab_end = 0;          // child slots reserved on the stack of level+1
 
-    // per-lane ray state.  The DDA (s, od, sx, c) runs ONE CELL AHEAD of the physics: it describes the next
-    // cell to be traversed, while SA / SB hold the segment whose absorber loads are in flight.
+    // per-lane ray state.  The DDA (s, od, sx, c) runs TWO CELLS AHEAD of the physics: it describes the next
+    // cell to be traversed, while two of SA / SB / SC hold the segments whose absorber loads are in flight.
     bool has = false;
     double s = 0.0, tau = 0.0, N = 0.0;
-    double d0 = 0, d1 = 0, d2 = 0, inv0 = 0, inv1 = 0, inv2 = 0, od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
-    IDX c = 0, cst0 = 0, cst1 = 0, cst2 = 0;       // cell (padded linear index) and its signed step per axis
+    double od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
+    IDX c = 0;                                     // cell (padded linear index)
     unsigned long long cnt = 0;                    // periodic box: steps left to the faces (3 x 21 bits)
-    SegDesc<IDX> SA, SB;
-    SA.split = SB.split = 0;
+    SegDesc<IDX> SA, SB, SC;
+    SA.split = SB.split = SC.split = 0;
 
     // G stage: describe the cell the DDA stands in (everything here is geometry: no loaded value is needed),
     // issue its absorber loads, and advance the DDA to the next cell.  A cell that meets the split criterion
@@ -267,9 +290,9 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         D.fc = 1.0;
         if (GEOM != 0) {
             const double s_m = fma(0.5, ds, s);                                   // = s + 0.5 ds (0.5 ds is exact)
-            double m0 = fma(s_m, d0, 0.5) - od0;
-            double m1 = fma(s_m, d1, 0.5) - od1;
-            double m2 = fma(s_m, d2, 0.5) - od2;
+            double m0 = fma(s_m, T.d[0][threadIdx.x], 0.5) - od0;
+            double m1 = fma(s_m, T.d[1][threadIdx.x], 0.5) - od1;
+            double m2 = fma(s_m, T.d[2][threadIdx.x], 0.5) - od2;
             // nearest face, first minimum in the order x-, x+, y-, y+, z-, z+ (ties inside an axis go to the
             // minus side, ties between axes to the earlier axis: the same choice as six sequential tests)
             const double t0 = 1.0 - m0, t1 = 1.0 - m1, t2 = 1.0 - m2;
@@ -305,10 +328,13 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         }
         // advance one cell (DEC: s = s_exit; s_a = ((o_a + [d_a > 0]) - 0.5) / d_a)
         s = s_exit;
-        if (ax == 0) { od0 += signed_one(inv0); sx0 = (od0 + signed_half(inv0)) * inv0; }
-        if (ax == 1) { od1 += signed_one(inv1); sx1 = (od1 + signed_half(inv1)) * inv1; }
-        if (ax == 2) { od2 += signed_one(inv2); sx2 = (od2 + signed_half(inv2)) * inv2; }
-        const IDX stp = ax == 0 ? cst0 : (ax == 1 ? cst1 : cst2);
+        const double iv = T.inv[ax][threadIdx.x];
+        const double one = signed_one(iv), half = signed_half(iv);
+        if (ax == 0) { od0 += one; sx0 = (od0 + half) * iv; }
+        if (ax == 1) { od1 += one; sx1 = (od1 + half) * iv; }
+        if (ax == 2) { od2 += one; sx2 = (od2 + half) * iv; }
+        const IDX ustp = ax == 0 ? (IDX)1 : (ax == 1 ? sy : sz);
+        const IDX stp = __double2hiint(iv) < 0 ? -ustp : ustp;                  // 1/d < 0: the ray moves down the axis
         if (PER) {
             const int sh = WRAP_BITS * ax;
             const int n_ax = ax == 0 ? A.nx : (ax == 1 ? A.ny : A.nz);
@@ -339,9 +365,9 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 ++n_seg;
                 const double dtau = (fabs(D.a_c) * sdx) * D.ds;
                 double pm, left, dN;
-                if (LUT) {
+                if constexpr (LUT) {
                     left = lut_q(A, tau + dtau);                                  // Q at the end of the segment
-                    dN = T.w[threadIdx.x] * (left - N);
+                    dN = T.w.v[threadIdx.x] * (left - N);
                 } else {
                     absorb_fraction(dtau, pm, left);
                     dN = N * (-pm);
@@ -378,7 +404,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         const unsigned m_exit = __ballot_sync(0xffffffffu, outcome == OUT_EXIT);
         const unsigned m_klmax = __ballot_sync(0xffffffffu, outcome == OUT_KILL_LMAX);
         if (lane == 0) {
-            n_split += __popc(m_split); n_ktau += __popc(m_ktau); n_exit += __popc(m_exit); n_klmax += __popc(m_klmax);
+            W.n_split[wid] += __popc(m_split); W.n_ktau[wid] += __popc(m_ktau); W.n_exit[wid] += __popc(m_exit);
+            W.n_klmax[wid] += __popc(m_klmax);
         }
         if (outcome == OUT_EXIT) T.esc[threadIdx.x] += rN;
         else if (outcome == OUT_KILL_TAU || outcome == OUT_KILL_LMAX) T.res[threadIdx.x] += rN;
@@ -387,6 +414,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             // first `rem` slots (a multiple of 4) finish the old slab and the rest start a new one: no slot is
             // wasted, so B marched rays push at most 4B children (+ one partly used slab per warp per launch)
             const int need = 4 * __popc(m_split);
+            long long slab_pos = W.slab_pos[wid], slab_end = W.slab_end[wid];
+            __syncwarp();
             const long long rem = slab_end - slab_pos;
             long long base = 0;
             if (need > rem) {
@@ -396,7 +425,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 if (base + CHILD_SLAB > A.pool.cap[level + 1]) {
                     if (lane == 0) A.ls->overflow = 1;
                     for (long long h = slab_pos + lane; h < slab_end; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
-                    slab_pos = slab_end = 0;
+                    if (lane == 0) W.slab_pos[wid] = W.slab_end[wid] = 0;
+                    __syncwarp();
                     return;
                 }
             }
@@ -415,6 +445,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             }
             if (need > rem) { slab_pos = base + (need - rem); slab_end = base + CHILD_SLAB; }
             else slab_pos += need;
+            if (lane == 0) { W.slab_pos[wid] = slab_pos; W.slab_end[wid] = slab_end; }
+            __syncwarp();
         }
     };
 
@@ -435,7 +467,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             if (mine) ikey = A.pool.key[r];
             const bool real = ikey != KEY_HOLE;
             const unsigned m_hole = __ballot_sync(0xffffffffu, mine && !real);
-            if (lane == 0) n_hole += __popc(m_hole);
+            if (lane == 0) W.n_hole[wid] += __popc(m_hole);
             double ts = 0.0, ttau = 0.0, tN = 0.0, e0 = 0.0, e1 = 0.0, e2 = 0.0, i0 = 0.0, i1 = 0.0, i2 = 0.0;
             IDX tc = 0;
             unsigned long long tcnt = 0;
@@ -481,7 +513,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 Q.d0[wid][e] = e0; Q.d1[wid][e] = e1; Q.d2[wid][e] = e2;
                 Q.inv0[wid][e] = i0; Q.inv1[wid][e] = i1; Q.inv2[wid][e] = i2;
                 Q.c[wid][e] = tc;
-                if (PER) Q.cnt[wid][e] = tcnt;
+                if constexpr (PER) Q.cnt.v[wid * 32 + e] = tcnt;
             }
             qhead = 0;
             qn = __popc(m_park);
@@ -499,18 +531,17 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 const int e = qhead + rank;
                 T.key[threadIdx.x] = Q.key[wid][e];
                 s = Q.s[wid][e]; tau = Q.tau[wid][e]; N = Q.N[wid][e];
-                if (LUT) { T.w[threadIdx.x] = N; N = lut_q(A, tau); }
-                d0 = Q.d0[wid][e]; d1 = Q.d1[wid][e]; d2 = Q.d2[wid][e];
-                inv0 = Q.inv0[wid][e]; inv1 = Q.inv1[wid][e]; inv2 = Q.inv2[wid][e];
+                if constexpr (LUT) { T.w.v[threadIdx.x] = N; N = lut_q(A, tau); }
+                const double d0 = Q.d0[wid][e], d1 = Q.d1[wid][e], d2 = Q.d2[wid][e];
+                const double inv0 = Q.inv0[wid][e], inv1 = Q.inv1[wid][e], inv2 = Q.inv2[wid][e];
+                T.d[0][threadIdx.x] = d0; T.d[1][threadIdx.x] = d1; T.d[2][threadIdx.x] = d2;
+                T.inv[0][threadIdx.x] = inv0; T.inv[1][threadIdx.x] = inv1; T.inv[2][threadIdx.x] = inv2;
                 c = Q.c[wid][e];
-                if (PER) cnt = Q.cnt[wid][e];
+                if constexpr (PER) cnt = Q.cnt.v[wid * 32 + e];
                 double q;
                 q = fma(s, d0, 0.5); od0 = floor(q); if (q == od0 && d0 < 0.0) od0 -= 1.0;
                 q = fma(s, d1, 0.5); od1 = floor(q); if (q == od1 && d1 < 0.0) od1 -= 1.0;
                 q = fma(s, d2, 0.5); od2 = floor(q); if (q == od2 && d2 < 0.0) od2 -= 1.0;
-                cst0 = d0 > 0.0 ? (IDX)1 : (IDX)-1;
-                cst1 = d1 > 0.0 ? sy : -sy;
-                cst2 = d2 > 0.0 ? sz : -sz;
                 sx0 = (od0 + signed_half(inv0)) * inv0;                        // ((o + [d > 0]) - 0.5) / d
                 sx1 = (od1 + signed_half(inv1)) * inv1;
                 sx2 = (od2 + signed_half(inv2)) * inv2;
@@ -518,6 +549,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 // pending segment = a null one (zero length, no deposit): the first pair of the march
                 // describes the real first cell; the null segment's zero-length tally is taken back here
                 SA.a_c = 0.0; SA.a_n = 0.0; SA.ds = 0.0; SA.fc = 1.0; SA.c = c; SA.cq = c; SA.split = 0;
+                SB = SA;
+                n_zero -= 1u;
                 n_zero -= 1u;
             }
             qhead += take;
@@ -528,22 +561,28 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             if (exhausted && qn == 0) break;                                      // nothing staged, nothing in flight
             continue;
         }
-        // ---- march: seg_round/2 pairs of cells per lane, then retire / refill --------------------------
+        // ---- march: seg_round/3 triples of cells per lane, then retire / refill ------------------------
         // Software pipeline: while the physics of one segment runs, the geometry stage has already issued
-        // the loads of the next one.  SA is the pending segment on entry and on exit of every pair.
+        // the loads of the next two (a gather has two iterations to arrive).
         int outcome = OUT_NONE;
-        for (int it = 0; it < seg_round; it += 2) {
+        for (int it = 0; it < seg_round; it += 3) {
             if (has && outcome == OUT_NONE) {
-                if (!SA.split) describe(SB);
+                // SA, SB pending (in that order) on entry and on exit.  A flagged segment (split / travel limit)
+                // stops the DDA: the descriptors behind it are not described, only marked, and never processed.
+                if (!SB.split) describe(SC); else SC.split = SB.split;
                 outcome = physics(SA);
                 if (outcome == OUT_NONE) {
-                    if (!SB.split) describe(SA);
+                    if (!SC.split) describe(SA); else SA.split = SC.split;
                     outcome = physics(SB);
+                    if (outcome == OUT_NONE) {
+                        if (!SA.split) describe(SB); else SB.split = SA.split;
+                        outcome = physics(SC);
+                    }
                 }
             }
         }
-        if (LUT) {
-            const double w = T.w[threadIdx.x];
+        if constexpr (LUT) {
+            const double w = T.w.v[threadIdx.x];
             retire(outcome, s, tau, w * (1.0 - N), w, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
         } else {
             retire(outcome, s, tau, N, N, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
@@ -551,7 +590,8 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         if (outcome != OUT_NONE) has = false;
     }
     // pad the unused tail of the last child slab
-    for (long long h = slab_pos + lane; h < slab_end; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
+    __syncwarp();
+    for (long long h = W.slab_pos[wid] + lane; h < W.slab_end[wid]; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
 
     // flush per-thread / per-warp tallies
     unsigned long long seg64 = n_seg, zero64 = n_zero;
@@ -568,11 +608,11 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         DevStats *ds = A.ds;
         if (seg64) atomicAdd(&ds->segments, seg64);
         if (zero64) atomicAdd(&ds->zero_len, zero64);
-        if (n_split) atomicAdd(&ds->split[level], (unsigned long long)n_split);
-        if (n_ktau) atomicAdd(&ds->killed_tau[level], (unsigned long long)n_ktau);
-        if (n_exit) atomicAdd(&ds->exited[level], (unsigned long long)n_exit);
-        if (n_klmax) atomicAdd(&ds->killed_lmax[level], (unsigned long long)n_klmax);
-        if (n_hole) atomicAdd(&ds->holes[level], (unsigned long long)n_hole);
+        if (W.n_split[wid]) atomicAdd(&ds->split[level], (unsigned long long)W.n_split[wid]);
+        if (W.n_ktau[wid]) atomicAdd(&ds->killed_tau[level], (unsigned long long)W.n_ktau[wid]);
+        if (W.n_exit[wid]) atomicAdd(&ds->exited[level], (unsigned long long)W.n_exit[wid]);
+        if (W.n_klmax[wid]) atomicAdd(&ds->killed_lmax[level], (unsigned long long)W.n_klmax[wid]);
+        if (W.n_hole[wid]) atomicAdd(&ds->holes[level], (unsigned long long)W.n_hole[wid]);
         if (esc != 0.0) atomicAdd(&ds->escaped, esc);
         if (res != 0.0) atomicAdd(&ds->residual, res);
         if (lost != 0.0) atomicAdd(&ds->lost, lost);

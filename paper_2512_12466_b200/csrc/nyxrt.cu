@@ -143,9 +143,9 @@ int effective_levels(const nyxrt_ctx *c) {
 uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, int staging) {
     Bump b{static_cast<char *>(base), 0};
     const long long n = max_sources > 0 ? max_sources : 1;
-    // the march's geometry stage runs one cell ahead of its box-exit test: a ray that is leaving may read
-    // (never use) up to two planes beyond the halo, so the absorber field has a guard band on both sides
-    const long long guard = 2 * ((long long)(c->g.nx + 2) * (c->g.ny + 2) + (c->g.nx + 2) + 4);
+    // the march's geometry stage runs two cells ahead of its box-exit test: a ray that is leaving may read
+    // (never use) up to three planes beyond the halo, so the absorber field has a guard band on both sides
+    const long long guard = 4 * ((long long)(c->g.nx + 2) * (c->g.ny + 2) + (c->g.nx + 2) + 4);
     c->absorber = b.take<double>(c->pcell + 2 * guard);
     if (c->absorber) c->absorber += guard;
     c->acc = b.take<double>(c->pcell);
@@ -220,7 +220,7 @@ void launch_march(const MarchArgs &a, bool idx64, bool per, int blocks, cudaStre
 
 template <typename K>
 cudaError_t setup_kernel(K kern, int *occ) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 32);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, MARCH_CARVEOUT);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, kern, MARCH_THREADS, MARCH_SMEM);
     return e;
 }
