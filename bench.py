@@ -38,6 +38,8 @@ def parse():
                     help="N > 1: shard the step by source (one all-reduce of the photon grid) instead of N replicas")
     ap.add_argument("--spectrum-teff", type=float, default=0.0,
                     help="trace with the tau_0 lookup table of a black body of this temperature [K] (default: monochromatic)")
+    ap.add_argument("--timestep-myr", type=float, default=0.0,
+                    help="time a whole RT timestep of this length (iterative RT<->ODE solve, nyxrt_timestep) instead of one RT step")
     ap.add_argument("--periodic", action="store_true", help="periodic box (default: BASELINE.json's open box)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -227,8 +229,26 @@ def main():
     if args.shard:
         tr.set_shard(rank, world)
 
+    class _TS:                                                     # timestep mode: the sum over the iterations
+        pass
+
     def step():
         # one RT step: fields of this step -> absorber field, sources -> catalogue, ray loop, finalise
+        if args.timestep_myr > 0:
+            tr.set_sources(pos, L, stream)
+            ode = nyxrt.make_ode(args.timestep_myr * 3.1557e13)
+            y0 = xHI.double() if xHI.dtype != torch.float64 else xHI
+            xe, xa, g_, h_, st1, ts = tr.timestep(ode, nH, y0, stream=stream)
+            out = _TS()
+            for name, _ in st1._fields_:
+                setattr(out, name, getattr(st1, name))
+            out.segments = ts.segments_total
+            out.kernel_launches = ts.kernel_launches
+            out.ms_march = st1.ms_march * ts.iterations           # per-launch events exist for the last trace only
+            out.march_launches = st1.march_launches * ts.iterations
+            out.timestep = dict(iterations=ts.iterations, converged=ts.converged, ms_rt=ts.ms_rt, ms_ode=ts.ms_ode,
+                                unconverged_cells=int(ts.unconverged_cells))
+            return out
         tr.set_fields(nH, xHI, stream)
         tr.set_sources(pos, L, stream)
         if not args.shard:
@@ -264,6 +284,8 @@ def main():
     ms = e0.elapsed_time(e1)
     clk = clocks.stop() if rank == 0 else None
     ms = max_over_ranks(ms, "cuda")
+    if args.timestep_myr > 0:
+        args.no_e2e = True
     if args.shard:
         seg_all = sum_over_ranks(seg, "cuda")                       # total work is fixed: strong scaling
         value = whole_job_rate(seg_all, ms, 1)
@@ -324,7 +346,7 @@ def main():
                                l2="inputs larger than L2 (fields + accumulator = %.1f GB), no flush"
                                   % ((2 * nH.numel() * nH.element_size() + 16 * nH.numel()) / 1e9),
                                multi_gpu="sharded by source, one all-reduce of the photon grid" if args.shard else "replicas only",
-                               periodic=bool(args.periodic),
+                               periodic=bool(args.periodic), timestep=getattr(st, "timestep", None),
                                spectrum=("black body %g K, tau_0 table 2^-20..2^12, 256 nodes per octave" % args.spectrum_teff)
                                if args.spectrum_teff > 0 else "monochromatic"),
                    rt_step_ms=ms / args.steps, march_ms_per_step=ms_march / args.steps,
