@@ -23,6 +23,11 @@ sys.path.insert(0, ROOT)
 
 ALGO_BYTES_PER_SEGMENT = {"f32": 48, "f64": 64}     # 4 field loads + 2 accumulator RMWs
 METRIC = "ray_cell_segments_per_s"
+# Secondary (ALU / issue) roof of the march kernel: one ray-cell costs 230 executed warp
+# instructions of which 76 are fp64 (profiles/r1_v12_march_config5.md); an fp64 warp instruction holds the
+# sub-partition's fp64 pipe for two cycles, so a warp-cell takes >= 230 + 76 issue cycles.
+ISSUE_CYCLES_PER_WARP_CELL = 306
+SM_COUNT, SCHEDULERS_PER_SM, LANES = 148, 4, 32
 
 
 def parse():
@@ -327,6 +332,13 @@ def main():
                     peak_source=peak_src,
                     note="achieved = %d B x segments / sum of march-launch durations (CUDA events around every "
                          "launch on the launching stream); DRAM traffic per launch: see profiles/" % bps)
+        sm_hz = 1e6 * float((clk or {}).get("sm_mhz") or 1965.0)
+        alu_peak = SM_COUNT * SCHEDULERS_PER_SM * sm_hz * LANES / ISSUE_CYCLES_PER_WARP_CELL
+        roof["alu"] = dict(bound="alu", achieved=seg / (ms_march * 1e-3), peak=alu_peak, unit="segments/s",
+                           frac=seg / (ms_march * 1e-3) / alu_peak,
+                           note="issue-slot roof of the march kernel: SMs x 4 schedulers x SM clock x 32 lanes / %d issue "
+                                "cycles per warp-cell (all lanes busy, no stall); the kernel is bound by this, not by HBM"
+                                % ISSUE_CYCLES_PER_WARP_CELL)
         tfile = os.path.join(ROOT, "profiles", "march_traffic.json")
         if os.path.exists(tfile):
             try:
