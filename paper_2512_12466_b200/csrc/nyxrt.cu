@@ -694,8 +694,14 @@ int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, co
             return fail(ctx, NYXRT_EINVAL, "set_spectrum: Q must be non-decreasing within [0, 1]");
     if (ctx->d_lut) cudaFree(ctx->d_lut);
     ctx->d_lut = nullptr;
-    CU(cudaMalloc(&ctx->d_lut, n * sizeof(double)));
-    CU(cudaMemcpy(ctx->d_lut, h_q, n * sizeof(double), cudaMemcpyHostToDevice));
+    double *d = nullptr;
+    CU(cudaMalloc(&d, n * sizeof(double)));
+    const cudaError_t ce = cudaMemcpy(d, h_q, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) {
+        cudaFree(d);
+        return fail(ctx, NYXRT_ECUDA, "set_spectrum: copy failed: %s", cudaGetErrorString(ce));
+    }
+    ctx->d_lut = d;
     ctx->lut_e_lo = e_lo; ctx->lut_e_hi = e_hi; ctx->lut_m = m; ctx->lut_n = n;
     ctx->lut_first = h_q[0];
     ctx->lut_last = h_q[n - 1];
