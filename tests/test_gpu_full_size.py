@@ -63,6 +63,47 @@ def test_config5_full_grid_sampled_sources(O, cfg5):
     print("config 5 full grid, %d sources: %d segments, worst relative Gamma error %.2e" % (N_SAMPLE, sg.segments, worst))
 
 
+def test_config5_full_grid_spectrum_table_in_two_shards(O, cfg5):
+    """The frequency-integrated flux (1e5 K black-body table) and the source-sharded path at full
+    size: the sample's catalogue is traced as two shards, the photon grids are added (the all-reduce) and
+    finalised; against the oracle with the same table, element by element on the full 1024^3 grid."""
+    pos, L = cfg5["src_pos"].numpy()[:N_SAMPLE], cfg5["src_L"].numpy()[:N_SAMPLE]
+    geom = (-20, 12, 6)
+    table = O.blackbody_table(1e5, *geom)
+    p = dict(cfg5["params"])
+    p["tau_max"] = 80.0
+    tr = nyxrt.Tracer(cfg5["shape"], cfg5["dx_cm"], p, field_dtype=cfg5["nH"].dtype, max_sources=N_SAMPLE)
+    try:
+        tr.set_spectrum(*geom, table)
+        tr.set_fields(cfg5["nH"], cfg5["xHI"])
+        tr.set_sources(pos, L)
+        total = torch.zeros(cfg5["shape"], dtype=torch.float64, device="cuda")
+        stats = []
+        for r in range(2):
+            tr.set_shard(r, 2)
+            ph, st = tr.trace_photons()
+            total += ph
+            stats.append(st)
+        del ph
+        gam, heat, absorbed = tr.finalise(total)
+        del total
+    finally:
+        tr.close()
+    sub = dict(cfg5)
+    sub["src_pos"], sub["src_L"] = cfg5["src_pos"][:N_SAMPLE], cfg5["src_L"][:N_SAMPLE]
+    try:
+        O.set_spectrum(*geom, table)
+        go, ho, so, co = run_oracle(O, sub, params=dict(tau_max=80.0))
+    finally:
+        O.set_spectrum()
+    for name in COUNTERS:
+        assert [a + b for a, b in zip(getattr(stats[0], name), getattr(stats[1], name))] == list(getattr(so, name)), name
+    assert stats[0].segments + stats[1].segments == so.segments and stats[0].segments > 0 and stats[1].segments > 0
+    worst = compare_slabs(gam, heat, go, ho, cfg5, params=dict(tau_max=80.0))
+    assert abs(absorbed - so.photons_absorbed) <= 1e-11 * so.photons_absorbed
+    print("config 5 full grid, spectrum table, 2 shards: %d segments, worst relative Gamma error %.2e" % (so.segments, worst))
+
+
 def test_config5_full_step_properties(cfg5):
     pos, L = cfg5["src_pos"].numpy(), cfg5["src_L"].numpy()
     gam, heat, st, cat = _trace(cfg5, pos, L)
