@@ -630,23 +630,26 @@ __global__ void prep_fields_kernel(const T *__restrict__ nH, const T *__restrict
                                    double *__restrict__ partial) {
     __shared__ double sh[256];
     double acc = 0.0;
-    const long long px = nx + 2, py = ny + 2, pz = nz + 2, ptot = px * py * pz;
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < ptot;
-         q += (long long)gridDim.x * blockDim.x) {
-        long long i = q % px - 1, j = (q / px) % py - 1, k = q / (px * py) - 1;
-        double v = -CUDART_INF;
-        const bool inside = i >= 0 && i < nx && j >= 0 && j < ny && k >= 0 && k < nz;
-        if (periodic) {                            // halo = image of the opposite side
-            i = (i + nx) % nx; j = (j + ny) % ny; k = (k + nz) % nz;
+    // one padded row (fixed j, k) per block iteration, threads along x: no division per cell, coalesced rows
+    const long long px = nx + 2, py = ny + 2, pz = nz + 2, nrow = py * pz;
+    for (long long row = blockIdx.x; row < nrow; row += gridDim.x) {
+        long long j = row % py - 1, k = row / py - 1;
+        const bool row_inside = j >= 0 && j < ny && k >= 0 && k < nz;
+        if (periodic) { j = (j + ny) % ny; k = (k + nz) % nz; }       // halo = image of the opposite side
+        const long long src = (k * ny + j) * nx, dst = row * px;
+        for (int ip = threadIdx.x; ip < (int)px; ip += blockDim.x) {
+            int i = ip - 1;
+            const bool inside = row_inside && i >= 0 && i < nx;
+            double v = -CUDART_INF;
+            if (periodic) i = i < 0 ? nx - 1 : (i >= nx ? 0 : i);
+            if (inside || periodic) {
+                const double n = (double)nH[src + i], x = (double)xHI[src + i];
+                v = n * x;
+                if (use_flag && !(n >= n_th)) v = -v;
+                if (inside) acc += 1.0 - x;
+            }
+            a[dst + ip] = v;
         }
-        if (inside || periodic) {
-            const long long t = (k * ny + j) * nx + i;
-            const double n = (double)nH[t], x = (double)xHI[t];
-            v = n * x;
-            if (use_flag && !(n >= n_th)) v = -v;
-            if (inside) acc += 1.0 - x;
-        }
-        a[q] = v;
     }
     sh[threadIdx.x] = acc;
     __syncthreads();
@@ -681,10 +684,11 @@ __global__ void finalise_kernel(double *__restrict__ gamma, double *__restrict__
                                 double *__restrict__ partial) {
     __shared__ double sh[256];
     double sum = 0.0;
-    const long long ncell = (long long)nx * ny * nz, px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2);
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < ncell;
-         t += (long long)gridDim.x * blockDim.x) {
-        const long long i = t % nx, j = (t / nx) % ny, k = t / ((long long)nx * ny);
+    const long long px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2), nrow = (long long)ny * nz;
+    for (long long row = blockIdx.x; row < nrow; row += gridDim.x)
+    for (int i = threadIdx.x; i < nx; i += blockDim.x) {             // one row (fixed j, k) per block iteration
+        const long long j = row % ny, k = row / ny;
+        const long long t = row * nx + i;
         const long long q = (k + 1) * pxy + (j + 1) * px + (i + 1);
         double ph = acc[q];
         if (periodic) {
@@ -722,10 +726,11 @@ __global__ void finalise_dense_kernel(double *__restrict__ gamma, double *__rest
                                       int ny, int nz, double V, double e_excess, double *__restrict__ partial) {
     __shared__ double sh[256];
     double sum = 0.0;
-    const long long ncell = (long long)nx * ny * nz, px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2);
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < ncell;
-         t += (long long)gridDim.x * blockDim.x) {
-        const long long i = t % nx, j = (t / nx) % ny, k = t / ((long long)nx * ny);
+    const long long px = nx + 2, pxy = (long long)(nx + 2) * (ny + 2), nrow = (long long)ny * nz;
+    for (long long row = blockIdx.x; row < nrow; row += gridDim.x)
+    for (int i = threadIdx.x; i < nx; i += blockDim.x) {             // one row (fixed j, k) per block iteration
+        const long long j = row % ny, k = row / ny;
+        const long long t = row * nx + i;
         const long long q = (k + 1) * pxy + (j + 1) * px + (i + 1);
         const double ph = photons[t];
         sum += ph;
