@@ -35,6 +35,7 @@ __global__ void ode_kernel(const double *__restrict__ gamma, const T *__restrict
         const double g = gamma[c], nh = (double)nH[c], y0 = y_begin[c], y_old = (double)y_avg[c];
         double yavg = y_old, yend = y0;
         for (int it = 0; it < o.inner_iter; ++it) {
+            const double yprev = yavg;
             const double ne = (1.0 - yavg) * nh;
             const double a_ion = g + ne * o.coll;
             const double a_rec = (ne * o.alpha) * o.clumping;
@@ -47,6 +48,7 @@ __global__ void ode_kernel(const double *__restrict__ gamma, const T *__restrict
             yavg = yeq + (y0 - yeq) * (-em1 / w);
             yend = yend < 0.0 ? 0.0 : (yend > 1.0 ? 1.0 : yend);
             yavg = yavg < 0.0 ? 0.0 : (yavg > 1.0 ? 1.0 : yavg);
+            if (yavg == yprev) break;        // a fixed point, bit for bit: the remaining iterations would repeat it
         }
         const T stored = (T)yavg;
         y_avg[c] = stored;
