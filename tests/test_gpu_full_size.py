@@ -143,6 +143,30 @@ def test_config5_full_step_properties(cfg5):
     assert abs(st2.photons_absorbed - st.photons_absorbed) <= BUDGET_RTOL * st.photons_emitted
 
 
+def test_config5_full_step_periodic_properties(cfg5):
+    """The full 10^6-source step in a PERIODIC box (the paper's production mode): ray-count
+    identities per level, photon budget, grid-side absorbed sum (which includes the shares folded back from the
+    halo), and more work than the open box (rays wrap instead of leaving)."""
+    pos, L = cfg5["src_pos"].numpy(), cfg5["src_L"].numpy()
+    gam, heat, st, cat = _trace(cfg5, pos, L, periodic=1)
+    assert st.spawned[0] == 12 * st.n_src_merged
+    for l in range(16):
+        assert st.spawned[l] == st.split[l] + st.killed_tau[l] + st.killed_lmax[l] + st.exited[l], l
+        if l < 15:
+            assert st.spawned[l + 1] == 4 * st.split[l], l
+    assert st.segments > 8.3 * 10 ** 11                      # the open box: 8.21e11
+    assert_budget(st, "gpu")
+    V = cfg5["dx_cm"] ** 3
+    nHI = cfg5["nH"].double() * cfg5["xHI"].double()
+    absorbed = float((gam * nHI).sum()) * V
+    assert abs(absorbed - st.photons_absorbed) <= 1e-10 * st.photons_absorbed
+    assert float(gam.min()) >= 0.0 and bool(torch.isfinite(gam).all())
+    # every face is lit from the other side: the boundary planes receive photons
+    for face in (gam[0], gam[-1], gam[:, 0], gam[:, -1], gam[:, :, 0], gam[:, :, -1]):
+        assert float(face.sum()) > 0.0
+    print("config 5 periodic: %d segments, %d merged sources" % (st.segments, st.n_src_merged))
+
+
 @pytest.mark.parametrize("config_id,n_sample", [(3, 40), (4, 3)])
 def test_configs_3_4_full_grid_sampled_sources(O, config_id, n_sample):
     """Configs 3 (256^3, merging off) and 4 (512^3, merging on), fp64 fields: the full grid, a sample of the
