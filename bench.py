@@ -339,10 +339,15 @@ def main():
                            note="issue-slot roof of the march kernel: SMs x 4 schedulers x SM clock x 32 lanes / %d issue "
                                 "cycles per warp-cell (all lanes busy, no stall); the kernel is bound by this, not by HBM"
                                 % ISSUE_CYCLES_PER_WARP_CELL)
-        tfile = os.path.join(ROOT, "profiles", "march_traffic.json")
+        tfile = os.path.join(ROOT, "profiles", "march_traffic.csv")     # measured by ncu, see profiles/*.md
         if os.path.exists(tfile):
             try:
-                roof["traffic"] = json.load(open(tfile)).get("dram_bytes_per_launch")
+                import csv
+                with open(tfile, newline="") as f:
+                    for row in csv.DictReader(f):
+                        if row.get("dram_bytes_per_launch"):
+                            roof["traffic"] = float(row["dram_bytes_per_launch"])
+                            break
             except (ValueError, OSError):
                 pass
         cpu = None
