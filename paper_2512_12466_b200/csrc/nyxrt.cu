@@ -32,6 +32,8 @@ struct SrcBufs {
     int *par, *lab_a, *lab_b, *bin_a, *bin_b;
     int4 *cell[2];
     double *L2[2], *r[2];
+    int4 *m_cell;                          // group members in group order (collapse)
+    double *m_L, *m_r;
     long long *ckey[2];
     int *bad;
     double *dirs;                          // shell sample directions, 12*4^samp_level
@@ -184,6 +186,9 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
         s.r[k] = b.take<double>(n);
         s.ckey[k] = b.take<long long>(n);
     }
+    s.m_cell = b.take<int4>(n);
+    s.m_L = b.take<double>(n);
+    s.m_r = b.take<double>(n);
     s.bad = b.take<int>(4);
     s.dirs = b.take<double>(3ull * 12ull << (2 * c->p.samp_level));
     s.cub_bytes = cub_temp_bytes(n);
@@ -256,7 +261,7 @@ int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     ctx->n_dedup = ctx->n_cat = 0;
     ctx->cat_sel = 0;
     if (n == 0) return NYXRT_OK;
-    ctx->n_aux_launches += do_merge ? 14 : 4;     // own kernels below (CUB launches not counted)
+    ctx->n_aux_launches += do_merge ? 16 : 4;     // own kernels below (CUB launches not counted)
     int key_bits = 1;
     while (((long long)1 << key_bits) < ctx->ncell) ++key_bits;
     size_t tb = s.cub_bytes;
@@ -311,8 +316,13 @@ int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     head_flags_int_kernel<<<nb, 256, 0, st>>>(s.lab_b, nd, s.flag);
     tb = s.cub_bytes;
     CU(cub::DeviceScan::InclusiveSum(s.cub_tmp, tb, s.flag, s.gid, nd, st));
-    collapse_kernel<<<nb, 256, 0, st>>>(s.lab_b, s.idx_b, s.flag, s.gid, nd, s.cell[0], s.L2[0], s.r[0], gd, s.cell[1],
-                                        s.L2[1], s.r[1], s.ckey[1]);
+    gather_members_kernel<<<nb, 256, 0, st>>>(s.idx_b, nd, s.cell[0], s.L2[0], s.r[0], s.m_cell, s.m_L, s.m_r);
+    CU(cudaMemsetAsync(s.bad + 1, 0, sizeof(int), st));               // number of large groups
+    collapse_kernel<<<nb, 256, 0, st>>>(s.lab_b, s.flag, s.gid, nd, s.m_cell, s.m_L, s.m_r, gd, s.cell[1],
+                                        s.L2[1], s.r[1], s.ckey[1], s.bin_a, s.bad + 1);
+    collapse_big_kernel<<<ctx->sm_count * 2, 32 * COLLAPSE_WARPS, 0, st>>>(s.lab_b, s.gid, nd, s.m_cell, s.m_L, s.m_r, gd,
+                                                                          s.cell[1], s.L2[1], s.r[1], s.ckey[1], s.bin_a,
+                                                                          s.bad + 1);
     int nm = 0;
     CU(cudaMemcpyAsync(&nm, s.gid + (nd - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));

@@ -150,6 +150,8 @@ __global__ void bin_kernel(const int4 *__restrict__ cell, long long n, int W, in
     idx[a] = (int)a;
 }
 
+constexpr int BIG_GROUP = 64;             // groups of this many members or more go to collapse_big_kernel
+
 __device__ __forceinline__ long long lower_bound_int(const int *v, long long n, int x) {
     long long lo = 0, hi = n;
     while (lo < hi) {
@@ -221,22 +223,42 @@ __global__ void head_flags_int_kernel(const int *__restrict__ key, long long n, 
     flag[t] = (t == 0 || key[t] != key[t - 1]) ? 1 : 0;
 }
 
+// members of all groups laid out contiguously in group order (the sort by label is stable, so members keep
+// their ascending catalogue order): collapse_kernel then streams them instead of chasing sidx -> cell / L / r
+__global__ void gather_members_kernel(const int *__restrict__ sidx, long long n, const int4 *__restrict__ cell,
+                                      const double *__restrict__ L, const double *__restrict__ rad,
+                                      int4 *__restrict__ m_cell, double *__restrict__ m_L, double *__restrict__ m_r) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    const int b = sidx[e];
+    m_cell[e] = cell[b];
+    m_L[e] = L[b];
+    m_r[e] = rad[b];
+}
+
 // one thread per group (members = a run of equal labels, ascending catalogue index): flux sum, max
-// radius, flux-weighted centroid, round, snap to the nearest member (first on ties) -- PAPER.md:378-387
-__global__ void collapse_kernel(const int *__restrict__ slabel, const int *__restrict__ sidx,
+// radius, flux-weighted centroid, round, snap to the nearest member (first on ties) -- PAPER.md:378-387.
+// cell / L / rad are the member arrays of gather_members_kernel (indexed like slabel).  The sums are
+// sequential in member order (DESIGN.md DEC); a percolating group of 10^5 members is one thread's loop.
+__global__ void collapse_kernel(const int *__restrict__ slabel,
                                 const int *__restrict__ flag, const int *__restrict__ gid_incl, long long n,
                                 const int4 *__restrict__ cell, const double *__restrict__ L,
                                 const double *__restrict__ rad, GridDims g, int4 *__restrict__ out_cell,
                                 double *__restrict__ out_L, double *__restrict__ out_r,
-                                long long *__restrict__ out_key) {
+                                long long *__restrict__ out_key, int *__restrict__ big_list, int *big_n) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n || !flag[t]) return;
     const int lab = slabel[t];
+    const long long end = lower_bound_int(slabel, n, lab + 1);       // labels are sorted: the run ends here
+    if (end - t >= BIG_GROUP) {                                      // a warp does it (collapse_big_kernel)
+        big_list[atomicAdd(big_n, 1)] = (int)t;
+        return;
+    }
     long long e = t;
     double F = 0.0, R = 0.0, n0 = 0.0, n1 = 0.0, n2 = 0.0;
-    const int4 ref = cell[sidx[t]];                // periodic: images nearest to the first member
-    for (; e < n && slabel[e] == lab; ++e) {
-        const int b = sidx[e];
+    const int4 ref = cell[t];                      // periodic: images nearest to the first member
+    for (; e < end; ++e) {
+        const long long b = e;
         const double l = L[b];
         const int4 c = cell[b];
         long long x0 = c.x, x1 = c.y, x2 = c.z;
@@ -254,20 +276,20 @@ __global__ void collapse_kernel(const int *__restrict__ slabel, const int *__res
     int4 oc;
     double oL, oR;
     if (e - t == 1) {
-        const int b = sidx[t];
+        const long long b = t;
         oc = cell[b]; oL = L[b]; oR = rad[b];
     } else {
         long long r0 = (long long)floor(n0 / F + 0.5), r1 = (long long)floor(n1 / F + 0.5),
                   r2 = (long long)floor(n2 / F + 0.5);
         if (g.periodic) { r0 = wrap_idx(r0, g.nx); r1 = wrap_idx(r1, g.ny); r2 = wrap_idx(r2, g.nz); }
         long long bestd = -1;
-        int best = -1;
+        long long best = -1;
         for (long long u = t; u < e; ++u) {
-            const int4 c = cell[sidx[u]];
+            const int4 c = cell[u];
             long long ex = c.x - r0, ey = c.y - r1, ez = c.z - r2;
             if (g.periodic) { ex = min_image(ex, g.nx); ey = min_image(ey, g.ny); ez = min_image(ez, g.nz); }
             const long long d2 = ex * ex + ey * ey + ez * ez;
-            if (best < 0 || d2 < bestd) { best = sidx[u]; bestd = d2; }
+            if (best < 0 || d2 < bestd) { best = u; bestd = d2; }
         }
         oc = cell[best]; oL = F; oR = R;
     }
@@ -276,6 +298,81 @@ __global__ void collapse_kernel(const int *__restrict__ slabel, const int *__res
     out_L[gid] = oL;
     out_r[gid] = oR;
     out_key[gid] = ((long long)oc.z * g.ny + oc.y) * g.nx + oc.x;
+}
+
+// Large groups (a percolating bubble can hold 10^5 sources): one warp per group.  The sums stay sequential in
+// member order (DESIGN.md DEC: they steer a rounding) -- lane 0 adds, the warp only stages 32 members at a time
+// in shared memory with coalesced loads; the snap (an integer minimum, first member on ties) is a warp reduction.
+constexpr int COLLAPSE_WARPS = 4;
+__global__ void __launch_bounds__(32 * COLLAPSE_WARPS)
+collapse_big_kernel(const int *__restrict__ slabel, const int *__restrict__ gid_incl, long long n,
+                    const int4 *__restrict__ cell, const double *__restrict__ L, const double *__restrict__ rad,
+                    GridDims g, int4 *__restrict__ out_cell, double *__restrict__ out_L, double *__restrict__ out_r,
+                    long long *__restrict__ out_key, const int *__restrict__ big_list, const int *big_n) {
+    __shared__ double sl[COLLAPSE_WARPS][32], sr[COLLAPSE_WARPS][32], s0[COLLAPSE_WARPS][32], s1[COLLAPSE_WARPS][32],
+        s2[COLLAPSE_WARPS][32];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int nbig = *big_n;
+    for (int w = blockIdx.x * COLLAPSE_WARPS + wid; w < nbig; w += gridDim.x * COLLAPSE_WARPS) {
+        const long long t = big_list[w];
+        const long long end = lower_bound_int(slabel, n, slabel[t] + 1);
+        const int4 ref = cell[t];
+        double F = 0.0, R = 0.0, n0 = 0.0, n1 = 0.0, n2 = 0.0;
+        for (long long base = t; base < end; base += 32) {
+            const long long u = base + lane;
+            if (u < end) {
+                const int4 c = cell[u];
+                long long x0 = c.x, x1 = c.y, x2 = c.z;
+                if (g.periodic) {
+                    x0 = ref.x + min_image(x0 - ref.x, g.nx);
+                    x1 = ref.y + min_image(x1 - ref.y, g.ny);
+                    x2 = ref.z + min_image(x2 - ref.z, g.nz);
+                }
+                sl[wid][lane] = L[u]; sr[wid][lane] = rad[u];
+                s0[wid][lane] = (double)x0; s1[wid][lane] = (double)x1; s2[wid][lane] = (double)x2;
+            }
+            __syncwarp();
+            if (lane == 0) {
+                const int m = (int)((end - base) < 32 ? (end - base) : 32);
+                for (int k = 0; k < m; ++k) {
+                    const double l = sl[wid][k];
+                    F = F + l;
+                    if (sr[wid][k] > R) R = sr[wid][k];
+                    n0 = n0 + l * s0[wid][k];
+                    n1 = n1 + l * s1[wid][k];
+                    n2 = n2 + l * s2[wid][k];
+                }
+            }
+            __syncwarp();
+        }
+        long long r0 = 0, r1 = 0, r2 = 0;
+        if (lane == 0) {
+            r0 = (long long)floor(n0 / F + 0.5); r1 = (long long)floor(n1 / F + 0.5); r2 = (long long)floor(n2 / F + 0.5);
+            if (g.periodic) { r0 = wrap_idx(r0, g.nx); r1 = wrap_idx(r1, g.ny); r2 = wrap_idx(r2, g.nz); }
+        }
+        r0 = __shfl_sync(0xffffffffu, r0, 0); r1 = __shfl_sync(0xffffffffu, r1, 0); r2 = __shfl_sync(0xffffffffu, r2, 0);
+        long long bestd = 0x7fffffffffffffffll, best = 0x7fffffffffffffffll;
+        for (long long u = t + lane; u < end; u += 32) {
+            const int4 c = cell[u];
+            long long ex = c.x - r0, ey = c.y - r1, ez = c.z - r2;
+            if (g.periodic) { ex = min_image(ex, g.nx); ey = min_image(ey, g.ny); ez = min_image(ez, g.nz); }
+            const long long d2 = ex * ex + ey * ey + ez * ez;
+            if (d2 < bestd) { bestd = d2; best = u; }                  // first minimum of this lane's members
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {                             // first minimum over the lanes
+            const long long od = __shfl_down_sync(0xffffffffu, bestd, o), ou = __shfl_down_sync(0xffffffffu, best, o);
+            if (od < bestd || (od == bestd && ou < best)) { bestd = od; best = ou; }
+        }
+        if (lane == 0) {
+            const int gid = gid_incl[t] - 1;
+            const int4 oc = cell[best];
+            out_cell[gid] = oc;
+            out_L[gid] = F;
+            out_r[gid] = R;
+            out_key[gid] = ((long long)oc.z * g.ny + oc.y) * g.nx + oc.x;
+        }
+    }
 }
 
 // gather a catalogue through a permutation (after the final sort by cell key)

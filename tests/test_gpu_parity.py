@@ -195,3 +195,22 @@ def test_error_paths():
     bad.periodic = 2
     with pytest.raises(nyxrt.NyxrtError):
         nyxrt.nyxrt_create(bad, nyxrt.make_params(**p))
+
+
+@pytest.mark.parametrize("periodic", [0, 1])
+def test_merge_large_groups(O, periodic):
+    """Fully ionised gas: every bubble reaches R_max and the bubbles percolate, so almost all sources collapse
+    into one group of thousands of members (collapse_big_kernel: one warp per large group, sums sequential in
+    member order) next to a few small ones; the catalogue must equal the oracle's bit for bit."""
+    cfg = synth.make(4, n=40, n_src=4000)
+    cfg["xHI"] = torch.full_like(cfg["xHI"], 1e-3)
+    rg = run_gpu(cfg, batch_rays=16384, periodic=periodic)
+    ro = run_oracle(O, cfg, periodic=periodic)
+    compare(rg, ro, cfg)
+    st = rg[2]
+    assert st.n_src_dedup > 1000 and st.n_src_merged < 40          # one giant group (and maybe a few loners)
+    cfgb = synth.make(4, n=40, n_src=4000, r_max=2.0)             # many groups of tens to hundreds of members
+    cfgb["xHI"] = torch.full_like(cfgb["xHI"], 1e-3)
+    rgb = run_gpu(cfgb, batch_rays=16384, periodic=periodic)
+    compare(rgb, run_oracle(O, cfgb, periodic=periodic), cfgb)
+    assert 10 < rgb[2].n_src_merged < rgb[2].n_src_dedup
