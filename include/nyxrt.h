@@ -1,7 +1,7 @@
 /*
  * nyxrt.h -- C ABI of the B200-native adaptive ray-tracing step (one RT step on the coarse grid) of
  * Nyx-RT, arxiv 2512.12466.  Citations are lines of /root/reference/PAPER.md ("PAPER.md:<line>");
- * readings R1..R27 and H1 of the paper's silent / garbled spots are listed in DESIGN.md.
+ * readings R1..R42 and H1 of the paper's silent / garbled spots are listed in DESIGN.md.
  *
  * The step ("Ray tracing loop", Figs. 1-2 at PAPER.md:120-124; Sec. 2.8 at 295-391):
  *   source dedup + sort -> [bubble radius -> merge] -> emit 12 HEALPix rays per source ->
@@ -84,6 +84,8 @@ typedef struct {
     uint64_t killed_lmax[NYXRT_MAXLEV];  /* rays filtered by l >= l_max                             */
     uint64_t segments;                   /* ray-cell segments of positive length (the work unit)    */
     uint64_t zero_len_segments;          /* cell crossings of zero length (edge / corner hits)      */
+    uint64_t neighbour_deposits;         /* segments whose nearest neighbour cell received a share
+                                            (Eq. 6 / 8): the second gather + deposit */
     uint64_t n_src_in, n_src_dedup, n_src_merged;
     uint64_t iterations;                 /* march launches (diagnostic; not part of parity)         */
     uint64_t peak_pool_rays;             /* max rays resident in the pool (diagnostic)              */
@@ -196,7 +198,8 @@ int nyxrt_step_host(nyxrt_ctx *ctx, const void *h_nH, const void *h_xHI, int64_t
                     const double *L, double *h_gamma_HI, double *h_heat, nyxrt_stats *h_stats);
 
 /* Parameters of one RT TIMESTEP (time integration, Eq. 3, inside the iterative nonlinear
- * solve, "following [23]"; monochromatic, the lookup table of PAPER.md:95 is not built). */
+ * solve, "following [23]").  The ray traces inside use whatever flux is configured: monochromatic
+ * by default, the tau_0 lookup table of PAPER.md:95 once nyxrt_set_spectrum has been called (R32). */
 typedef struct {
     double  dt_s;              /* timestep [s], > 0                                                  */
     double  alpha_cm3_s;       /* recombination coefficient alpha_H(T) of Eq. 3 (2.59e-13 at 1e4 K)  */

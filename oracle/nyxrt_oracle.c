@@ -78,6 +78,7 @@ typedef struct {
     uint64_t spawned[ORC_MAXLEV], split[ORC_MAXLEV], killed_tau[ORC_MAXLEV], exited[ORC_MAXLEV],
              killed_lmax[ORC_MAXLEV];
     uint64_t segments, zero_len_segments;
+    uint64_t neighbour_deposits;   /* segments whose nearest neighbour received a share (Eq. 6 / 8) */
     uint64_t n_src_in, n_src_dedup, n_src_merged;
     double   photons_emitted, photons_absorbed, photons_escaped, photons_residual, photons_lost;
 } orc_stats;
@@ -609,6 +610,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
                 if (T->heat) T->heat[c] += p->e_excess_erg * fc * dN / T->V;       /* H1 */
                 long double dep = (long double)(fc * dN);
                 if (cn >= 0) {
+                    st->neighbour_deposits++;
                     double fn = (1.0 - fc) * (a_c / a_n);              /* Eq. 6 / Eq. 8: f_c' */
                     T->gamma[cn] += fn * gC;
                     if (T->heat) T->heat[cn] += p->e_excess_erg * (1.0 - fc) * dN / T->V;
@@ -740,8 +742,8 @@ int orc_sizeof_seg(void) { return (int)sizeof(orc_seg); }
 /* nonlinear solve (Sec. 2.4), "following the approach of [23]" (C2-Ray,        */
 /* Mellema et al. 2006): fix x, ray-trace for Gamma (orc_step above); fix Gamma, integrate Eq. 3  */
 /* over dt with the semi-analytic, time-averaged solution; iterate until convergence.             */
-/* Monochromatic (constant sigma): the frequency-integrated lookup table of PAPER.md:95 is not    */
-/* built (the paper prints no source spectrum).  Readings R32-R36.                    */
+/* The ray traces inside use the flux that is configured: monochromatic (constant sigma) by       */
+/* default, the tau_0 lookup table of PAPER.md:95 after orc_set_spectrum (R32).  Readings R32-R36. */
 
 typedef struct {
     double  dt_s;             /* timestep                                                       */

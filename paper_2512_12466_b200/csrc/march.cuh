@@ -41,6 +41,7 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->emit_n = 0;
     ls->batch = 0;
     ls->fetch = 0;
+    if (ls->overflow) ls->done = 1;                          // a pool overflow ends the loop: EOVERFLOW, never garbage
     if (ls->done) return;
     const long long B = ls->batch_rays;
     int pick = -1;
@@ -77,7 +78,7 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->level = pick;
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
-    ls->seg_round = ls->tune_seg_round > 0 ? ls->tune_seg_round : (pick < 2 ? 3 : 21);
+    ls->seg_round = pick < 2 ? 3 : 21;
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
@@ -246,7 +247,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
 
     T.esc[threadIdx.x] = 0.0;
     T.res[threadIdx.x] = 0.0;
-    unsigned int n_seg = 0, n_zero = 0;
+    unsigned int n_seg = 0, n_zero = 0, n_nbr = 0;
     double lost = 0.0;
     if (lane == 0) {
         W.slab_pos[wid] = W.slab_end[wid] = 0;
@@ -377,6 +378,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                     if (GEOM == 3) {
                         if (D.a_n > 0.0) {                                        // in the box, absorber > 0, n_H >= n_th
                             fc = D.fc;
+                            ++n_nbr;
                             atomicAdd(acc + D.cq, (1.0 - fc) * dN);
                         }
                     } else if (GEOM == 1 || GEOM == 4) {
@@ -594,12 +596,13 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     for (long long h = W.slab_pos[wid] + lane; h < W.slab_end[wid]; h += 32) A.pool.key[A.pool.off[level + 1] + h] = KEY_HOLE;
 
     // flush per-thread / per-warp tallies
-    unsigned long long seg64 = n_seg, zero64 = n_zero;
+    unsigned long long seg64 = n_seg, zero64 = n_zero, nbr64 = n_nbr;
     double esc = T.esc[threadIdx.x], res = T.res[threadIdx.x];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         seg64 += __shfl_xor_sync(0xffffffffu, seg64, o);
         zero64 += __shfl_xor_sync(0xffffffffu, zero64, o);
+        nbr64 += __shfl_xor_sync(0xffffffffu, nbr64, o);
         esc += __shfl_xor_sync(0xffffffffu, esc, o);
         res += __shfl_xor_sync(0xffffffffu, res, o);
         lost += __shfl_xor_sync(0xffffffffu, lost, o);
@@ -608,6 +611,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
         DevStats *ds = A.ds;
         if (seg64) atomicAdd(&ds->segments, seg64);
         if (zero64) atomicAdd(&ds->zero_len, zero64);
+        if (nbr64) atomicAdd(&ds->nbr_deposits, nbr64);
         if (W.n_split[wid]) atomicAdd(&ds->split[level], (unsigned long long)W.n_split[wid]);
         if (W.n_ktau[wid]) atomicAdd(&ds->killed_tau[level], (unsigned long long)W.n_ktau[wid]);
         if (W.n_exit[wid]) atomicAdd(&ds->exited[level], (unsigned long long)W.n_exit[wid]);

@@ -48,7 +48,6 @@ struct nyxrt_ctx {
     nyxrt_params p;
     char err[512];
     int sm_count, march_blocks, nlev;
-    int tune_seg_round;                    // NYXRT_SEG_ROUND (tuning knob, 0 = scheduler's choice)
     long long ncell;
     // workspace
     void *ws;
@@ -142,12 +141,17 @@ int effective_levels(const nyxrt_ctx *c) {
     return nlev;
 }
 
+// the march's geometry stage runs ahead of its box-exit test: a ray that is leaving may read (never use) up to
+// three planes plus one neighbour offset beyond the halo; the absorber field carries this many guard cells on
+// both sides, and the cell index type must be able to address them
+long long guard_cells(const nyxrt_grid &g) { return 4 * ((long long)(g.nx + 2) * (g.ny + 2) + (g.nx + 2) + 4); }
+
 uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, int staging) {
     Bump b{static_cast<char *>(base), 0};
     const long long n = max_sources > 0 ? max_sources : 1;
     // the march's geometry stage runs two cells ahead of its box-exit test: a ray that is leaving may read
     // (never use) up to three planes beyond the halo, so the absorber field has a guard band on both sides
-    const long long guard = 4 * ((long long)(c->g.nx + 2) * (c->g.ny + 2) + (c->g.nx + 2) + 4);
+    const long long guard = guard_cells(c->g);
     c->absorber = b.take<double>(c->pcell + 2 * guard);
     if (c->absorber) c->absorber += guard;
     c->acc = b.take<double>(c->pcell);
@@ -373,7 +377,7 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     ctx->shard_rank = 0;
     ctx->shard_world = 1;
     ctx->pcell = (long long)(g.nx + 2) * (g.ny + 2) * (g.nz + 2);
-    ctx->idx64 = ctx->pcell >= (1ll << 31);
+    ctx->idx64 = ctx->pcell + guard_cells(g) >= (1ll << 31);      // the guard band must be addressable too
     const double PI = 0x1.921fb54442d18p+1;
     for (int l = 0; l < MAXLEV; ++l) {
         ctx->r2_split[l] = std::ldexp(3.0 / (PI * p.n_min_ray), 2 * l);   // Eq. 4
@@ -411,7 +415,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     }
     ctx->sm_count = prop.multiProcessorCount;
     ctx->march_blocks = ctx->sm_count * (occ > 0 ? occ : 1);
-    if (const char *v = getenv("NYXRT_SEG_ROUND")) ctx->tune_seg_round = atoi(v);
     *out = ctx;
     return NYXRT_OK;
 }
@@ -434,13 +437,11 @@ void nyxrt_destroy(nyxrt_ctx *ctx) {
 
 int nyxrt_workspace_bytes(const nyxrt_ctx *cctx, int64_t max_sources, int64_t batch_rays, int32_t host_staging,
                           uint64_t *bytes) {
-    nyxrt_ctx *ctx = const_cast<nyxrt_ctx *>(cctx);
-    if (!ctx || !bytes || max_sources < 0 || batch_rays < 0 || max_sources >= (1ll << 30))
-        return fail(ctx, NYXRT_EINVAL, "workspace_bytes: bad argument");
-    if (ctx->ws) return fail(ctx, NYXRT_ESTATE, "workspace_bytes: query before set_workspace");
-    const long long B = batch_rays ? batch_rays : default_batch(ctx);
-    if (B < 32) return fail(ctx, NYXRT_EINVAL, "workspace_bytes: batch_rays must be >= 32");
-    *bytes = layout(ctx, nullptr, max_sources, B, host_staging);
+    if (!cctx || !bytes || max_sources < 0 || batch_rays < 0 || max_sources >= (1ll << 30)) return NYXRT_EINVAL;
+    const long long B = batch_rays ? batch_rays : default_batch(cctx);
+    if (B < 32) return NYXRT_EINVAL;
+    nyxrt_ctx scratch = *cctx;                    // a pure query: the layout is laid out on a copy
+    *bytes = layout(&scratch, nullptr, max_sources, B, host_staging);
     return NYXRT_OK;
 }
 
@@ -452,7 +453,8 @@ int nyxrt_set_workspace(nyxrt_ctx *ctx, void *d_ws, uint64_t bytes, int64_t max_
     const long long B = batch_rays ? batch_rays : default_batch(ctx);
     if (B < 32) return fail(ctx, NYXRT_EINVAL, "set_workspace: batch_rays must be >= 32");
     ctx->ws = nullptr;
-    const uint64_t need = layout(ctx, nullptr, max_sources, B, host_staging);
+    nyxrt_ctx scratch = *ctx;
+    const uint64_t need = layout(&scratch, nullptr, max_sources, B, host_staging);
     if (bytes < need) return fail(ctx, NYXRT_ENOMEM, "set_workspace: %llu bytes given, %llu needed",
                                   (unsigned long long)bytes, (unsigned long long)need);
     layout(ctx, d_ws, max_sources, B, host_staging);
@@ -550,7 +552,6 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     memset(ctx->h_ls, 0, sizeof(LoopState));
     ctx->h_ls->n_cat = n_local;
     ctx->h_ls->batch_rays = ctx->batch_rays;
-    ctx->h_ls->tune_seg_round = ctx->tune_seg_round;
     CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
     MarchArgs a;
     memset(&a, 0, sizeof a);
@@ -638,6 +639,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         }
         hs->segments = d.segments;
         hs->zero_len_segments = d.zero_len;
+        hs->neighbour_deposits = d.nbr_deposits;
         hs->n_src_in = (uint64_t)ctx->n_src;
         hs->n_src_dedup = (uint64_t)ctx->n_dedup;
         hs->n_src_merged = (uint64_t)ctx->n_cat;

@@ -108,20 +108,20 @@ __global__ void radius_kernel(const int4 *__restrict__ cell, long long n, const 
 
 // ---- union-find, smaller index wins (so the root of a component is its smallest member) -------------
 // par[x] <= x always, so following parents strictly descends until a root (par[r] == r).  Reads bypass
-// L1 (volatile): other threads hook roots concurrently with atomicCAS.  Path compression only rewrites
-// non-roots with one of their ancestors, hooking only rewrites roots, so the two never collide.
+// L1 (volatile): other threads hook roots concurrently with atomicCAS.  Two passes: walk to the root, then
+// point every node of the walked path at it.  The second pass only rewrites non-roots with one of their
+// ancestors and hooking only rewrites roots, so the two never collide; a concurrent hook may make `root`
+// a non-root meanwhile, which only means the path is compressed to an ancestor instead of the new root.
 __device__ __forceinline__ int uf_find(int *par, int a) {
     volatile int *vp = par;
-    int curr = vp[a];
-    if (curr != a) {
-        int prev = a, next;
-        while (curr > (next = vp[curr])) {
-            vp[prev] = next;
-            prev = curr;
-            curr = next;
-        }
+    int root = a;
+    for (int up = vp[root]; up != root; up = vp[root]) root = up;
+    while (a != root) {
+        const int up = vp[a];
+        if (up > root) vp[a] = root;
+        a = up < root ? root : up;
     }
-    return curr;
+    return root;
 }
 
 __device__ __forceinline__ void uf_unite(int *par, int a, int b) {

@@ -32,7 +32,6 @@ struct LoopState {
     int done;
     int overflow;
     int seg_round;                       // cells marched per round, between two retire / pop passes
-    int tune_seg_round;                  // > 0: overrides the scheduler's choice (tuning knob)
     unsigned long long iterations, peak_pool;
     unsigned long long fetch;            // next unclaimed ray of the current batch (chunks of FETCH_CHUNK)
 };
@@ -40,7 +39,7 @@ struct LoopState {
 struct DevStats {
     unsigned long long spawned[MAXLEV], split[MAXLEV], killed_tau[MAXLEV], exited[MAXLEV], killed_lmax[MAXLEV];
     unsigned long long holes[MAXLEV];   // filler slots popped at level l (slab padding; not rays)
-    unsigned long long segments, zero_len;
+    unsigned long long segments, zero_len, nbr_deposits;
     double escaped, residual, lost;
     double absorbed;                     // finalise: sum over cells
     double emitted;

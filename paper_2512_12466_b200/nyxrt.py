@@ -41,7 +41,7 @@ class nyxrt_stats(C.Structure):
     _fields_ = [("spawned", C.c_uint64 * MAXLEV), ("split", C.c_uint64 * MAXLEV),
                 ("killed_tau", C.c_uint64 * MAXLEV), ("exited", C.c_uint64 * MAXLEV),
                 ("killed_lmax", C.c_uint64 * MAXLEV),
-                ("segments", C.c_uint64), ("zero_len_segments", C.c_uint64),
+                ("segments", C.c_uint64), ("zero_len_segments", C.c_uint64), ("neighbour_deposits", C.c_uint64),
                 ("n_src_in", C.c_uint64), ("n_src_dedup", C.c_uint64), ("n_src_merged", C.c_uint64),
                 ("iterations", C.c_uint64), ("peak_pool_rays", C.c_uint64),
                 ("photons_emitted", C.c_double), ("photons_absorbed", C.c_double),

@@ -75,6 +75,7 @@ def compare(res_gpu, res_or, cfg, params=None):
     for name in COUNTERS:
         assert list(getattr(sg, name)) == list(getattr(so, name)), (name, list(getattr(sg, name)), list(getattr(so, name)))
     assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    assert sg.neighbour_deposits == so.neighbour_deposits
     # rates
     err = np.abs(gg - go)
     bad = err > RTOL * np.abs(go) + ATOL

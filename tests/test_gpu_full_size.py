@@ -56,6 +56,7 @@ def test_config5_full_grid_sampled_sources(O, cfg5):
     for name in COUNTERS:
         assert list(getattr(sg, name)) == list(getattr(so, name)), name
     assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    assert sg.neighbour_deposits == so.neighbour_deposits
     assert sg.segments > 10 ** 7 and max(l for l in range(16) if sg.spawned[l]) >= 9
     worst = compare_slabs(gam, heat, go, ho, cfg5)
     assert_budget(sg, "gpu")
@@ -181,6 +182,7 @@ def test_configs_3_4_full_grid_sampled_sources(O, config_id, n_sample):
     for name in COUNTERS:
         assert list(getattr(sg, name)) == list(getattr(so, name)), name
     assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    assert sg.neighbour_deposits == so.neighbour_deposits
     worst = compare_slabs(gam, heat, go, ho, cfg)
     assert_budget(sg, "gpu")
     assert_budget(so, "oracle")
@@ -214,6 +216,7 @@ def test_64bit_cell_index_path(O, periodic):
     for name in COUNTERS:
         assert list(getattr(sg, name)) == list(getattr(so, name)), name
     assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    assert sg.neighbour_deposits == so.neighbour_deposits
     assert (sum(sg.exited) > 0) == (periodic == 0) and sum(sg.killed_tau) > 0 and sg.segments > 10 ** 6
     if periodic:
         assert float(gam[0, 0, 0]) > 0.0 and float(gam[-1, -1, 0]) > 0.0   # lit through the faces

@@ -43,7 +43,7 @@ class Sum:
     def __init__(self, stats, absorbed):
         for name in COUNTERS:
             setattr(self, name, [sum(getattr(s, name)[l] for s in stats) for l in range(16)])
-        for name in ("segments", "zero_len_segments"):
+        for name in ("segments", "zero_len_segments", "neighbour_deposits"):
             setattr(self, name, sum(getattr(s, name) for s in stats))
         for name in ("photons_emitted", "photons_escaped", "photons_residual", "photons_lost"):
             setattr(self, name, sum(getattr(s, name) for s in stats))

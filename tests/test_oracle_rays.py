@@ -152,6 +152,14 @@ def test_budget_and_grid_sum(O):
     assert abs(tot - ab) <= 1e-12 * ab
     # heating reading H1: heat = e_excess * photons absorbed per unit volume
     assert abs(float(heat.sum()) * V - 2e-11 * ab) <= 1e-12 * 2e-11 * ab
+    # ... PER CELL: for a monochromatic source heat[c] = e_excess n_HI[c] Gamma[c], because
+    # both grids receive the same photons (f_c dN in the cell, (1 - f_c) dN in the neighbour), Gamma divided by
+    # the receiving cell's n_HI V (Eq. 6 / 8's factor a_abs / a'_abs) and the heating by V alone
+    nHI = a * x
+    lit = gam > 0
+    assert lit.sum() > 1000
+    assert np.all(np.abs(heat[lit] - 2e-11 * nHI[lit] * gam[lit]) <= 1e-12 * heat[lit])
+    assert np.all(heat[~lit] == 0.0)
     assert np.all(gam[(a * x) == 0.0] == 0.0)
     # per level bookkeeping identities
     for l in range(15):
@@ -213,7 +221,9 @@ def test_deposit_shares_eq5_to_8(O):
     x[0, 1, 2] = 0.0
     n_th = 5e-4
     src = (2, 3, 2)
-    g, p, a, x, gam, heat, st, log = uniform_case(O, n, None, None, src, L=1e49, dx=5e19, fields=(a, x), n_th=n_th)
+    e_ex = 3e-11
+    g, p, a, x, gam, heat, st, log = uniform_case(O, n, None, None, src, L=1e49, dx=5e19, fields=(a, x), n_th=n_th,
+                                                   e_excess_erg=e_ex)
     org = np.array(src, float) + 0.5
     V = g.dx_cm ** 3
     photons = np.zeros((n, n, n))
@@ -268,8 +278,15 @@ def test_deposit_shares_eq5_to_8(O):
         else:
             assert r["nb_face"] == -1
     assert n_nb > 100 and n_th_block > 10 and n_edge_block > 10 and n_tie < 0.1 * len(log)
+    assert st.neighbour_deposits == n_nb                    # the counter of Eq. 6 / 8 deposits
     expect = np.divide(photons, a * x * V, out=np.zeros_like(photons), where=(a * x) > 0)
     assert np.allclose(gam, expect, rtol=1e-12, atol=0)
+    # heating (reading H1): e_excess per photon absorbed, per unit volume -- f_c dN of it in the cell,
+    # (1 - f_c) dN in the logged neighbour.  `photons` was rebuilt above from the log with exactly that split, so
+    # a share put in the wrong cell (all of it in c, or f_c and 1 - f_c swapped) fails here.
+    assert n_nb > 100 and np.count_nonzero(photons) > 50
+    assert np.allclose(heat, e_ex * photons / V, rtol=1e-12, atol=0)
+    assert np.array_equal(heat == 0.0, photons == 0.0)
 
 
 @pytest.mark.parametrize("mode,conserves", [(0, True), (1, False), (2, True), (3, True), (4, False)])
