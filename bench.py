@@ -45,7 +45,6 @@ def parse():
                     help="trace with the tau_0 lookup table of a black body of this temperature [K] (default: monochromatic)")
     ap.add_argument("--timestep-myr", type=float, default=0.0,
                     help="time a whole RT timestep of this length (iterative RT<->ODE solve, nyxrt_timestep) instead of one RT step")
-    ap.add_argument("--march-path", type=int, default=0, help="nyxrt_params.march_path (0 = automatic)")
     ap.add_argument("--periodic", action="store_true", help="periodic box (default: BASELINE.json's open box)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -222,7 +221,6 @@ def main():
     cfg, pos, L = make_workload(args, "cuda")
     nH, xHI = cfg["nH"], cfg["xHI"]
     fdt = "f32" if nH.dtype == torch.float32 else "f64"
-    cfg["params"]["march_path"] = args.march_path
     tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], cfg["params"], field_dtype=nH.dtype, max_sources=len(L),
                       batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local,
                       periodic=1 if args.periodic else 0)

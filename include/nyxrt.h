@@ -72,8 +72,7 @@ typedef struct {
     int32_t merge;             /* 0 off, 1 on, 2 automerge                           */
     int32_t n_min_samples;     /* N_min of PAPER.md:317                                             */
     int32_t samp_level;        /* HEALPix level of the shell sample pattern, 12*4^level dirs (R6)   */
-    int32_t march_path;        /* 0 = automatic (bundles in an open box, per-ray kernel in a periodic one),
-                                  1 = per-ray kernel, 2 = bundles (open box only); same results either way */
+    int32_t reserved;          /* 0                                                                 */
 } nyxrt_params;
 
 /* Filled by nyxrt_trace (host memory).  Per-level arrays are indexed by HEALPix level l. */

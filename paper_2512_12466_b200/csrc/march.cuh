@@ -36,9 +36,7 @@ constexpr int MARCH_CARVEOUT = 40;       // preferred shared-memory carve-out [%
 //   2. if sources remain, top level 0 up with 12 rays per source, then 1. again; else
 //   3. the shallowest non-empty level (drain).
 // With caps of 2B (level 0) and 5B + slab slack (deeper levels) no stack can overflow.
-// PER_SRC: pool entries a source starts with (12 rays, or 3 quads of 4 rays); POOL: RayPool or QuadPool.
-template <int PER_SRC, typename POOL>
-__global__ void sched_kernel(LoopState *ls, DevStats *ds, POOL pool, int nlev) {
+__global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     ls->emit_n = 0;
     ls->batch = 0;
@@ -50,14 +48,14 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, POOL pool, int nlev) {
     for (int l = nlev - 1; l >= 0; --l)
         if (ls->count[l] >= B) { pick = l; break; }
     if (pick < 0 && ls->src_next < ls->n_cat) {
-        long long room = (pool.cap[0] - ls->count[0]) / PER_SRC;
+        long long room = (pool.cap[0] - ls->count[0]) / 12;
         long long k = ls->n_cat - ls->src_next;
         if (k > room) k = room;
         if (k > 0) {
             ls->emit_src = ls->src_next;
             ls->emit_n = k;
             ls->emit_slot = pool.off[0] + ls->count[0];
-            ls->count[0] += PER_SRC * k;
+            ls->count[0] += 12 * k;
             ls->src_next += k;
         }
         if (ls->count[0] >= B) pick = 0;
@@ -82,8 +80,7 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, POOL pool, int nlev) {
     ls->batch = b;
     ls->seg_round = pick < 2 ? 3 : 21;
     ls->iterations += 1;
-    if (PER_SRC == 12) ds->spawned[pick] += (unsigned long long)b;   // rays: every slot is popped exactly once (holes subtracted
-                                                                     // later); bundles count their rays in the march
+    ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
 
 // ---------------------------------------------------------------------------------------------------

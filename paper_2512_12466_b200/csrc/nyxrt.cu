@@ -16,7 +16,6 @@
 
 #include "../../include/nyxrt.h"
 #include "march.cuh"
-#include "bundle.cuh"
 #include "sources.cuh"
 #include "timestep.cuh"
 
@@ -60,12 +59,6 @@ struct nyxrt_ctx {
     long long pcell;                       // padded cell count
     bool idx64;                            // padded grid needs 64-bit cell indices
     RayPool pool;
-    QuadPool qp;                           // shared-geometry path (open box): the same batch in quads of 4 rays
-    bool use_bundles;
-    int bundle_blocks;
-    long long batch_bundles;
-    void *sort_tmp;
-    size_t sort_bytes;
     LoopState *ls;
     DevStats *ds;
     SrcBufs sb;
@@ -173,36 +166,10 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
         c->pool.cap[l] = l < c->nlev ? (l == 0 ? 2 * B : 5 * B + (long long)CHILD_SLAB * c->march_blocks * MARCH_WARPS) : 0;
         total += c->pool.cap[l];
     }
-    if (!c->use_bundles) {
-        c->pool.key = b.take<uint64_t>(total);
-        c->pool.s = b.take<double>(total);
-        c->pool.tau = b.take<double>(total);
-        c->pool.N = b.take<double>(total);
-    } else {
-        // the same bound in quads (4 rays): a batch of Bq quads pushes at most 4 Bq children (allocated compactly)
-        const long long Bb = (B + 3) / 4;
-        long long tb = 0;
-        for (int l = 0; l < MAXLEV; ++l) {
-            c->qp.off[l] = tb;
-            c->qp.cap[l] = l < c->nlev ? (l == 0 ? 2 * Bb + 3 : 5 * Bb) : 0;
-            tb += c->qp.cap[l];
-        }
-        c->qp.key = b.take<uint32_t>(tb);
-        c->qp.src = b.take<uint32_t>(tb);
-        c->qp.s = b.take<double>(tb);
-        c->qp.tau = b.take<double>(tb);
-        c->qp.N = b.take<double>(tb);
-        c->qp.key_in = b.take<uint64_t>(Bb);
-        c->qp.key_out = b.take<uint64_t>(Bb);
-        c->qp.val_in = b.take<uint32_t>(Bb);
-        c->qp.val_out = b.take<uint32_t>(Bb);
-        size_t sb = 0;
-        cub::DeviceRadixSort::SortPairs(nullptr, sb, (uint64_t *)nullptr, (uint64_t *)nullptr, (uint32_t *)nullptr,
-                                        (uint32_t *)nullptr, (int)Bb);
-        c->sort_bytes = sb + 256;
-        c->sort_tmp = b.take<char>(c->sort_bytes);
-        c->batch_bundles = Bb;
-    }
+    c->pool.key = b.take<uint64_t>(total);
+    c->pool.s = b.take<double>(total);
+    c->pool.tau = b.take<double>(total);
+    c->pool.N = b.take<double>(total);
     SrcBufs &s = c->sb;
     s.pos = b.take<double>(3 * n);
     s.L = b.take<double>(n);
@@ -289,25 +256,6 @@ double bb_absorbed(double x0, double tau, bool with_abs) {
 }
 
 int geom_template(int mode) { return mode == 2 ? 3 : mode; }
-
-template <int GEOM, bool LUT>
-void launch_bundles(const MarchArgs &a, bool idx64, int blocks, cudaStream_t st) {
-    if (idx64) bundle_march_kernel<GEOM, long long, LUT, BUNDLE_RMAX><<<blocks, BUNDLE_THREADS, 0, st>>>(a);
-    else bundle_march_kernel<GEOM, int, LUT, BUNDLE_RMAX><<<blocks, BUNDLE_THREADS, 0, st>>>(a);
-}
-
-template <typename K>
-cudaError_t setup_bundle_kernel(K kern, int *occ) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 25);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ, kern, BUNDLE_THREADS, 0);
-    return e;
-}
-
-template <int GEOM, bool LUT>
-cudaError_t setup_bundles(bool idx64, int *occ) {
-    return idx64 ? setup_bundle_kernel(bundle_march_kernel<GEOM, long long, LUT, BUNDLE_RMAX>, occ)
-                 : setup_bundle_kernel(bundle_march_kernel<GEOM, int, LUT, BUNDLE_RMAX>, occ);
-}
 
 // ---- source pass: dedup + sort, optional radius + merge -------------------------------------------
 int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
@@ -418,7 +366,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     if (!(g.dx_cm > 0.0) || !(g.pos_unit_cm > 0.0) || (g.periodic != 0 && g.periodic != 1)) return NYXRT_EINVAL;
     if (!(p.sigma_cm2 > 0.0) || !(p.n_min_ray > 0.0) || !(p.tau_max > 0.0)) return NYXRT_EINVAL;
     if (p.level_max < 0 || p.level_max > 13 || p.geom_mode < 0 || p.geom_mode > 4) return NYXRT_EINVAL;
-    if (p.march_path < 0 || p.march_path > 2 || (p.march_path == 2 && g.periodic)) return NYXRT_EINVAL;
     if (p.merge < 0 || p.merge > 2 || p.samp_level < 0 || p.samp_level > 8 || !(p.delta_r > 0.0)) return NYXRT_EINVAL;
     if (!(p.r_max >= 0.0) || !(p.f_ov >= 0.0)) return NYXRT_EINVAL;
     nyxrt_ctx *ctx = new (std::nothrow) nyxrt_ctx();
@@ -437,7 +384,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
         ctx->K[l] = std::ldexp(std::sqrt(PI / 3.0), -l);                  // sqrt(4 pi / (12 4^l))
     }
     ctx->nlev = effective_levels(ctx);
-    ctx->use_bundles = p.march_path == 2;
     cudaError_t e = cudaSetDevice(g.device);
     cudaDeviceProp prop;
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, g.device);
@@ -462,21 +408,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
             }
         }
     }
-    int occ_b = 0;
-    if (e == cudaSuccess && ctx->use_bundles) {
-        switch (geom_template(p.geom_mode)) {
-            case 0: e = setup_bundles<0, false>(ctx->idx64, &occ_b); break;
-            case 1: e = setup_bundles<1, false>(ctx->idx64, &occ_b); break;
-            case 4: e = setup_bundles<4, false>(ctx->idx64, &occ_b); break;
-            default: {
-                int occ_lut = 0;
-                e = setup_bundles<3, true>(ctx->idx64, &occ_lut);
-                if (e == cudaSuccess) e = setup_bundles<3, false>(ctx->idx64, &occ_b);
-                if (occ_lut < occ_b) occ_b = occ_lut;
-                break;
-            }
-        }
-    }
     if (e != cudaSuccess) {
         // no CUDA device / wrong architecture: there is no fallback
         nyxrt_destroy(ctx);
@@ -484,7 +415,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     }
     ctx->sm_count = prop.multiProcessorCount;
     ctx->march_blocks = ctx->sm_count * (occ > 0 ? occ : 1);
-    ctx->bundle_blocks = ctx->sm_count * (occ_b > 0 ? occ_b : 1);
     *out = ctx;
     return NYXRT_OK;
 }
@@ -621,7 +551,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
     memset(ctx->h_ls, 0, sizeof(LoopState));
     ctx->h_ls->n_cat = n_local;
-    ctx->h_ls->batch_rays = ctx->use_bundles ? ctx->batch_bundles : ctx->batch_rays;
+    ctx->h_ls->batch_rays = ctx->batch_rays;
     CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
     MarchArgs a;
     memset(&a, 0, sizeof a);
@@ -630,8 +560,6 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     a.cat_cell = s.cell[0];
     a.cat_L = s.L2[0];
     a.pool = ctx->pool;
-    a.qp = ctx->qp;
-    a.order = nullptr;
     a.ls = ctx->ls;
     a.ds = ctx->ds;
     a.nx = ctx->g.nx; a.ny = ctx->g.ny; a.nz = ctx->g.nz;
@@ -660,49 +588,10 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     const int emit_blocks = ctx->sm_count * 4;
     int chunk = 8;
     long long n_launch = 0;
-    // bundles: a batch is sorted by pixel block so that bundles of different sources that share their geometry
-    // sit next to each other (pointless with one source: every pixel block then holds one bundle)
-    const bool sort_batch = ctx->use_bundles && n_local > 1;
-    int sort_bits = 1;
-    if (ctx->use_bundles) {
-        const long long max_key = 12ll << (2 * (ctx->nlev > 1 ? ctx->nlev - 2 : 0));   // parent pixels of the deepest level
-        while ((1ll << sort_bits) <= max_key) ++sort_bits;
-        if (sort_batch) a.order = ctx->qp.val_out;
-    }
-    int rank_bits = 1;
-    if (sort_batch) {
-        // rank of every catalogue source along a Morton curve (cells >> shift: at most 10 bits per axis)
-        const long long nc = ctx->n_cat;
-        while ((1ll << rank_bits) < nc) ++rank_bits;
-        int shift = 0, nmax = ctx->g.nx > ctx->g.ny ? ctx->g.nx : ctx->g.ny;
-        if (ctx->g.nz > nmax) nmax = ctx->g.nz;
-        while ((nmax >> shift) > 1024) ++shift;
-        SrcBufs &sw = ctx->sb;
-        morton_kernel<<<blocks_for(nc, 256), 256, 0, st>>>(s.cell[0], nc, shift, sw.bin_a, sw.idx_a);
-        size_t tb = sw.cub_bytes;
-        CU(cub::DeviceRadixSort::SortPairs(sw.cub_tmp, tb, sw.bin_a, sw.bin_b, sw.idx_a, sw.idx_b, (int)nc, 0, 30, st));
-        rank_kernel<<<blocks_for(nc, 256), 256, 0, st>>>(sw.idx_b, nc, (uint32_t *)sw.flag);
-        a.qp.src_rank = (const uint32_t *)sw.flag;
-        ctx->n_aux_launches += 2;
-    }
-    int launches_per_iter = 3;
     for (;;) {
         for (int i = 0; i < chunk; ++i) {
-            if (ctx->use_bundles) {
-                sched_kernel<3, QuadPool><<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->qp, ctx->nlev);
-                bundle_emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->qp, s.L2[0], ctx->shard_rank, ctx->shard_world);
-                if (sort_batch) {
-                    bundle_keys_kernel<<<ctx->sm_count * 2, 256, 0, st>>>(ctx->ls, a.qp, ctx->batch_bundles, rank_bits,
-                                                                          1ull << (sort_bits + rank_bits));
-                    size_t tb = ctx->sort_bytes;
-                    CU(cub::DeviceRadixSort::SortPairs(ctx->sort_tmp, tb, ctx->qp.key_in, ctx->qp.key_out, ctx->qp.val_in,
-                                                       ctx->qp.val_out, (int)ctx->batch_bundles, 0, sort_bits + rank_bits + 1, st));
-                    launches_per_iter = 4;
-                }
-            } else {
-                sched_kernel<12, RayPool><<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev);
-                emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0], ctx->shard_rank, ctx->shard_world);
-            }
+            sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev);
+            emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0], ctx->shard_rank, ctx->shard_world);
             if (n_launch + 1 > ctx->mev_cap / 2) {                       // grow the event pool
                 const long long cap = ctx->mev_cap ? 2 * ctx->mev_cap : 1024;
                 cudaEvent_t *m = (cudaEvent_t *)realloc(ctx->mev, cap * sizeof(cudaEvent_t));
@@ -712,17 +601,6 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
                 ctx->mev_cap = cap;
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
-            if (ctx->use_bundles) {
-                switch (gt) {
-                    case 0: launch_bundles<0, false>(a, ctx->idx64, ctx->bundle_blocks, st); break;
-                    case 1: launch_bundles<1, false>(a, ctx->idx64, ctx->bundle_blocks, st); break;
-                    case 4: launch_bundles<4, false>(a, ctx->idx64, ctx->bundle_blocks, st); break;
-                    default:
-                        if (lut) launch_bundles<3, true>(a, ctx->idx64, ctx->bundle_blocks, st);
-                        else launch_bundles<3, false>(a, ctx->idx64, ctx->bundle_blocks, st);
-                        break;
-                }
-            } else
             switch (gt) {
                 case 0: launch_march<0, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
                 case 1: launch_march<1, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
@@ -759,9 +637,6 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
             hs->spawned[l] = d.spawned[l] - d.holes[l]; hs->split[l] = d.split[l]; hs->killed_tau[l] = d.killed_tau[l];
             hs->exited[l] = d.exited[l]; hs->killed_lmax[l] = d.killed_lmax[l];
         }
-#ifdef NYXRT_DIAG
-        fprintf(stderr, "DIAG rounds %llu tasks %llu quads %llu warp-steps %llu slot-steps %llu lane-steps(any alive, per 2 steps) %llu segments %llu zero %llu\n", d.dg_rounds, d.dg_tasks, d.dg_quads, d.dg_steps, d.dg_slotsteps, d.dg_lanesteps, d.segments, d.zero_len);
-#endif
         hs->segments = d.segments;
         hs->zero_len_segments = d.zero_len;
         hs->neighbour_deposits = d.nbr_deposits;
@@ -769,7 +644,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         hs->n_src_dedup = (uint64_t)ctx->n_dedup;
         hs->n_src_merged = (uint64_t)ctx->n_cat;
         hs->iterations = ctx->h_ls->iterations;
-        hs->peak_pool_rays = ctx->h_ls->peak_pool * (ctx->use_bundles ? 4ull : 1ull);
+        hs->peak_pool_rays = ctx->h_ls->peak_pool;
         hs->photons_emitted = n_local ? ctx->h_scalars[2] : 0.0;
         hs->photons_absorbed = ctx->h_scalars[1];
         hs->photons_escaped = d.escaped;
@@ -788,7 +663,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         }
         hs->ms_march = (float)ms;
         hs->march_launches = (uint64_t)live;
-        hs->kernel_launches = (uint64_t)(launches_per_iter * n_launch) + ctx->n_aux_launches;
+        hs->kernel_launches = (uint64_t)(3 * n_launch) + ctx->n_aux_launches;
     }
     return NYXRT_OK;
 }

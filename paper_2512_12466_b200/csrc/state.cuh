@@ -21,20 +21,6 @@ struct RayPool {
     long long cap[MAXLEV];               // slots of level l
 };
 
-// The quad store (bundle.cuh): one stack of quads per HEALPix level.  A quad = the four children of one split
-// (PAPER.md:197): rays of one source in the pixels 4 key .. 4 key + 3 that share the distance travelled, the
-// optical depth and the photon share at birth: 32 bytes per quad, 8 per ray.  Level 0: keys 0, 1, 2 per source.
-struct QuadPool {
-    uint32_t *key;                       // parent pixel (nested index at level - 1)
-    uint32_t *src;                       // catalogue index of the source
-    double *s, *tau, *N;                 // distance [cells], optical depth, photons/s per child ray
-    long long off[MAXLEV];               // first slot of level l
-    long long cap[MAXLEV];               // slots of level l
-    uint64_t *key_in, *key_out;          // sort of a batch by (key, rank of the source along a space-filling curve)
-    uint32_t *val_in, *val_out;
-    const uint32_t *src_rank;            // [catalogue index] -> rank
-};
-
 // Loop control, written by sched_kernel and read by emit/march (no host round trip per iteration).
 struct LoopState {
     long long count[MAXLEV];             // rays on the stack of level l
@@ -57,9 +43,6 @@ struct DevStats {
     double escaped, residual, lost;
     double absorbed;                     // finalise: sum over cells
     double emitted;
-#ifdef NYXRT_DIAG
-    unsigned long long dg_rounds, dg_tasks, dg_quads, dg_steps, dg_slotsteps, dg_lanesteps;
-#endif
 };
 
 constexpr uint64_t KEY_HOLE = ~0ull;     // filler slot (end of a warp's child slab)
@@ -74,8 +57,6 @@ struct MarchArgs {
     const int4 *cat_cell;                // (i, j, k, 0) per catalogue source
     const double *cat_L;
     RayPool pool;
-    QuadPool qp;
-    const uint32_t *order;               // quads: batch positions sorted by key (null: stack order)
     LoopState *ls;
     DevStats *ds;
     int nx, ny, nz, level_max;

@@ -34,7 +34,7 @@ class nyxrt_params(C.Structure):
                 ("delta_r", C.c_double), ("r_max", C.c_double), ("f_ov", C.c_double), ("x_th", C.c_double),
                 ("f_req", C.c_double), ("eps", C.c_double),
                 ("level_max", C.c_int32), ("geom_mode", C.c_int32), ("merge", C.c_int32),
-                ("n_min_samples", C.c_int32), ("samp_level", C.c_int32), ("march_path", C.c_int32)]
+                ("n_min_samples", C.c_int32), ("samp_level", C.c_int32), ("reserved", C.c_int32)]
 
 
 class nyxrt_stats(C.Structure):
