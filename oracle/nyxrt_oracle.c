@@ -653,16 +653,20 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
     }
 }
 
-/* gamma, heat: [nz][ny][nx] double, overwritten.  heat may be NULL.  log may be NULL.
+/* gamma, heat: [nz][ny][nx] double; heat may be NULL.  zero != 0: overwritten; zero == 0: the deposits are ADDED
+   to what the grids hold and the counters to *st (Gamma is a sum over sources: a catalogue can be
+   traced slice by slice, or by several processes whose grids are added afterwards).  log may be NULL.
    *log_n_out (may be NULL) receives the number of segments that WOULD have been logged. */
-int orc_trace(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
-              int64_t n_cat, const int32_t *cell, const double *L, double *gamma, double *heat,
-              orc_stats *st, orc_seg *log, int64_t log_cap, int64_t *log_n_out) {
+static int trace_catalogue(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
+                           int64_t n_cat, const int32_t *cell, const double *L, double *gamma, double *heat,
+                           orc_stats *st, orc_seg *log, int64_t log_cap, int64_t *log_n_out, int zero) {
     if (p->level_max < 0 || p->level_max >= ORC_MAXLEV - 1 || !(p->n_min_ray > 0.0)) return ORC_EINVAL;
     if (p->geom_mode < 0 || p->geom_mode > 4) return ORC_EINVAL;
     int64_t ncell = (int64_t)g->nx * g->ny * g->nz;
-    memset(gamma, 0, (size_t)ncell * sizeof *gamma);
-    if (heat) memset(heat, 0, (size_t)ncell * sizeof *heat);
+    if (zero) {
+        memset(gamma, 0, (size_t)ncell * sizeof *gamma);
+        if (heat) memset(heat, 0, (size_t)ncell * sizeof *heat);
+    }
     tracer T;
     memset(&T, 0, sizeof T);
     T.g = g; T.p = p; T.nH = nH; T.xHI = xHI; T.gamma = gamma; T.heat = heat; T.st = st;
@@ -684,14 +688,38 @@ int orc_trace(const orc_grid *g, const orc_params *p, const void *nH, const void
         emitted += (long double)L[a];
         for (int64_t pix = 0; pix < 12; ++pix) trace_ray(&T, 0, pix, 0.0, 0.0);   /* PAPER.md:111 */
     }
-    st->photons_emitted = (double)emitted;
-    st->photons_absorbed = (double)T.absorbed;
-    st->photons_escaped = (double)T.escaped;
-    st->photons_residual = (double)T.residual;
-    st->photons_lost = (double)T.lost;
+    if (zero) {
+        st->photons_emitted = (double)emitted;
+        st->photons_absorbed = (double)T.absorbed;
+        st->photons_escaped = (double)T.escaped;
+        st->photons_residual = (double)T.residual;
+        st->photons_lost = (double)T.lost;
+    } else {
+        st->photons_emitted += (double)emitted;
+        st->photons_absorbed += (double)T.absorbed;
+        st->photons_escaped += (double)T.escaped;
+        st->photons_residual += (double)T.residual;
+        st->photons_lost += (double)T.lost;
+    }
     if (log_n_out) *log_n_out = T.log_n;
     return ORC_OK;
 }
+
+int orc_trace(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
+              int64_t n_cat, const int32_t *cell, const double *L, double *gamma, double *heat,
+              orc_stats *st, orc_seg *log, int64_t log_cap, int64_t *log_n_out) {
+    return trace_catalogue(g, p, nH, xHI, n_cat, cell, L, gamma, heat, st, log, log_cap, log_n_out, 1);
+}
+
+/* the same, accumulating into gamma / heat / *st (which the caller zeroes once) */
+int orc_trace_add(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
+                  int64_t n_cat, const int32_t *cell, const double *L, double *gamma, double *heat, orc_stats *st) {
+    return trace_catalogue(g, p, nH, xHI, n_cat, cell, L, gamma, heat, st, NULL, 0, NULL, 0);
+}
+
+/* the source pass of orc_step alone: dedup + sort, and bubble radii + merge when merging is on */
+int orc_catalogue(const orc_grid *g, const orc_params *p, const void *xHI, int64_t n_src, const double *pos,
+                  const double *L, orc_stats *st, int32_t *cat_cell, double *cat_L, double *cat_r, int64_t *n_cat);
 
 /* mean ionised fraction over all cells (automerge trigger, PAPER.md:311, 424) */
 double orc_mean_ionised(const orc_grid *g, const void *xHI) {
@@ -702,10 +730,8 @@ double orc_mean_ionised(const orc_grid *g, const void *xHI) {
 }
 
 /* The whole step.  cat_* have room for n_src entries; *n_cat receives the catalogue length. */
-int orc_step(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
-             int64_t n_src, const double *pos, const double *L,
-             double *gamma, double *heat, orc_stats *st,
-             int32_t *cat_cell, double *cat_L, double *cat_r, int64_t *n_cat) {
+int orc_catalogue(const orc_grid *g, const orc_params *p, const void *xHI, int64_t n_src, const double *pos,
+                  const double *L, orc_stats *st, int32_t *cat_cell, double *cat_L, double *cat_r, int64_t *n_cat) {
     memset(st, 0, sizeof *st);
     int64_t nd = 0;
     int rc = orc_prepare_sources(g, n_src, pos, L, cat_cell, cat_L, &nd);
@@ -731,7 +757,16 @@ int orc_step(const orc_grid *g, const orc_params *p, const void *nH, const void 
     }
     st->n_src_merged = (uint64_t)nm;
     *n_cat = nm;
-    return orc_trace(g, p, nH, xHI, nm, cat_cell, cat_L, gamma, heat, st, NULL, 0, NULL);
+    return ORC_OK;
+}
+
+int orc_step(const orc_grid *g, const orc_params *p, const void *nH, const void *xHI,
+             int64_t n_src, const double *pos, const double *L,
+             double *gamma, double *heat, orc_stats *st,
+             int32_t *cat_cell, double *cat_L, double *cat_r, int64_t *n_cat) {
+    int rc = orc_catalogue(g, p, xHI, n_src, pos, L, st, cat_cell, cat_L, cat_r, n_cat);
+    if (rc) return rc;
+    return orc_trace(g, p, nH, xHI, *n_cat, cat_cell, cat_L, gamma, heat, st, NULL, 0, NULL);
 }
 
 int orc_sizeof_stats(void) { return (int)sizeof(orc_stats); }

@@ -209,6 +209,33 @@ def step(g, p, nH, xHI, pos, L, want_heat=True):
     return gamma, heat, st, (cc[:m].copy(), cL[:m].copy(), cr[:m].copy())
 
 
+def catalogue(g, p, xHI, pos, L):
+    """The source pass alone (dedup + sort, bubble radii + merge when merging is on).
+    Returns (stats with the n_src_* fields, (cat_cell, cat_L, cat_r))."""
+    xHI = _field(g, xHI)
+    pos = np.ascontiguousarray(pos, dtype=np.float64).reshape(-1, 3)
+    L = np.ascontiguousarray(L, dtype=np.float64)
+    n = len(L)
+    st = Stats()
+    cc = np.zeros((max(n, 1), 3), np.int32)
+    cL = np.zeros(max(n, 1))
+    cr = np.zeros(max(n, 1))
+    ncat = C.c_int64(0)
+    _chk(lib().orc_catalogue(C.byref(g), C.byref(p), _ptr(xHI), C.c_int64(n), _ptr(pos), _ptr(L), C.byref(st),
+                             _ptr(cc), _ptr(cL), _ptr(cr), C.byref(ncat)), "catalogue")
+    m = ncat.value
+    return st, (cc[:m].copy(), cL[:m].copy(), cr[:m].copy())
+
+
+def trace_add(g, p, nH, xHI, cell, L, gamma, heat, st):
+    """orc_trace of a slice of the catalogue, ADDED to gamma / heat (numpy fp64 grids; heat may be None) and to
+    the counters of st.  nH / xHI must already have the grid's dtype and shape (no copy is made)."""
+    cell = np.ascontiguousarray(cell, np.int32).reshape(-1, 3)
+    L = np.ascontiguousarray(L, np.float64)
+    _chk(lib().orc_trace_add(C.byref(g), C.byref(p), _ptr(nH), _ptr(xHI), C.c_int64(len(L)), _ptr(cell), _ptr(L),
+                             _ptr(gamma), _ptr(heat) if heat is not None else None, C.byref(st)), "trace_add")
+
+
 def mean_ionised(g, xHI):
     return lib().orc_mean_ionised(C.byref(g), _ptr(_field(g, xHI)))
 

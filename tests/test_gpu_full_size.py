@@ -16,7 +16,8 @@ import pytest
 import torch
 
 from paper_2512_12466_b200 import nyxrt, synth
-from parity import BUDGET_RTOL, COUNTERS, assert_budget, compare_slabs, run_oracle
+from parity import (BUDGET_RTOL, COUNTERS, assert_budget, compare_slabs, compare_slabs_sum, run_oracle,
+                    run_oracle_parallel)
 
 pytestmark = pytest.mark.gpu
 
@@ -168,26 +169,61 @@ def test_config5_full_step_periodic_properties(cfg5):
     print("config 5 periodic: %d segments, %d merged sources" % (st.segments, st.n_src_merged))
 
 
-@pytest.mark.parametrize("config_id,n_sample", [(3, 40), (4, 3)])
-def test_configs_3_4_full_grid_sampled_sources(O, config_id, n_sample):
-    """Configs 3 (256^3, merging off) and 4 (512^3, merging on), fp64 fields: the full grid, a sample of the
-    source list the oracle finishes in seconds, element by element."""
+def _host_procs(bytes_per_proc):
+    """Worker processes for the oracle: the host's cores, capped by what its memory holds."""
+    import os
+    import psutil
+    p = os.cpu_count() or 1
+    return max(1, min(p, int(0.6 * psutil.virtual_memory().available // bytes_per_proc)))
+
+
+@pytest.mark.parametrize("config_id,n_sample,want_heat", [(3, 0, True), (4, 120, True), (5, 1500, False)])
+def test_configs_3_4_5_full_grid_parallel_oracle(O, config_id, n_sample, want_heat):
+    """Cell-by-cell parity at full grid size against the oracle run on all host cores (P
+    single-threaded oracle processes over disjoint chunks of the sorted catalogue, grids and counters added).
+    Config 3 (256^3, merging off): ALL 10^4 sources.  Config 4 (512^3, merging on) and config 5 (1024^3 fp32,
+    merging on): the first n_sample sources of the list -- the whole step (dedup, radii, merge, trace) on them;
+    a full config-4/5 step is 6.4e11 / 8.2e11 segments, days of host time.  Config 5 compares Gamma only (the
+    heating grids of 8 workers would not fit the host; heat = e_excess n_HI Gamma is checked on the device)."""
+    import time
     cfg = synth.make(config_id, device="cuda")
-    pos, L = cfg["src_pos"].numpy()[:n_sample], cfg["src_L"].numpy()[:n_sample]
-    gam, heat, sg, cg = _trace(cfg, pos, L)
+    if config_id == 5 and torch.cuda.mem_get_info()[1] < 100e9:
+        pytest.skip("needs the B200's memory")
+    n_sample = n_sample or len(cfg["src_L"])
     sub = dict(cfg)
     sub["src_pos"], sub["src_L"] = cfg["src_pos"][:n_sample], cfg["src_L"][:n_sample]
-    go, ho, so, co = run_oracle(O, sub)
-    assert np.array_equal(cg[0], co[0]) and np.array_equal(cg[1], co[1]) and np.array_equal(cg[2], co[2])
-    for name in COUNTERS:
-        assert list(getattr(sg, name)) == list(getattr(so, name)), name
-    assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
-    assert sg.neighbour_deposits == so.neighbour_deposits
-    worst = compare_slabs(gam, heat, go, ho, cfg)
-    assert_budget(sg, "gpu")
-    assert_budget(so, "oracle")
-    print("config %d full grid, %d sources: %d segments, worst relative Gamma error %.2e"
-          % (config_id, n_sample, sg.segments, worst))
+    pos, L = sub["src_pos"].numpy(), sub["src_L"].numpy()
+    gam, heat, sg, cg = _trace(cfg, pos, L)
+    ncell = int(np.prod(cfg["shape"]))
+    n_proc = _host_procs(ncell * 8 * (2 if want_heat else 1) + 2 ** 28)
+    t0 = time.perf_counter()
+    osum, co = run_oracle_parallel(O, sub, n_proc, want_heat=want_heat, chunk=8 if config_id == 3 else 1)
+    wall = time.perf_counter() - t0
+    try:
+        so = osum.stats
+        assert np.array_equal(cg[0], co[0]) and np.array_equal(cg[1], co[1]) and np.array_equal(cg[2], co[2])
+        for f in ("n_src_in", "n_src_dedup", "n_src_merged"):
+            assert getattr(sg, f) == getattr(so, f), f
+        for name in COUNTERS:
+            assert list(getattr(sg, name)) == list(getattr(so, name)), name
+        assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+        assert sg.neighbour_deposits == so.neighbour_deposits
+        worst = compare_slabs_sum(gam, heat if want_heat else None, osum, cfg)
+        if not want_heat:
+            nHI = cfg["nH"].double() * cfg["xHI"].double()
+            h_ref = cfg["params"]["e_excess_erg"] * nHI * gam
+            assert bool(((heat - h_ref).abs() <= 1e-12 * h_ref).all())
+        assert_budget(sg, "gpu")
+        assert_budget(so, "oracle")
+        for f in ("photons_emitted", "photons_absorbed", "photons_escaped", "photons_residual"):
+            a, b = getattr(sg, f), getattr(so, f)
+            assert abs(a - b) <= 1e-11 * so.photons_emitted, (f, a, b)
+    finally:
+        osum.close()
+    print("config %d full grid, %d of %d sources (%d merged): %d segments; oracle on %d processes: %.1f s wall, "
+          "%.3g segments/s aggregate, %.3g per core; worst relative Gamma error %.2e"
+          % (config_id, n_sample, len(cfg["src_L"]), sg.n_src_merged, sg.segments, osum.n_proc, wall,
+             sg.segments / wall, sg.segments / max(osum.cpu_seconds, 1e-9), worst))
 
 
 @pytest.mark.parametrize("periodic", [0, 1])
@@ -224,3 +260,34 @@ def test_64bit_cell_index_path(O, periodic):
     assert float(gam[-1, -1, -1]) > 0.0                       # the far corner cell (largest index) was lit
     assert_budget(sg, "gpu")
     print("64-bit index path: %d segments, worst relative Gamma error %.2e" % (sg.segments, worst))
+
+
+def test_guard_band_needs_64bit_indices(O):
+    """the padded grid itself has fewer than 2^31 cells, but the guard band behind the last halo plane
+    (which a leaving ray's look-ahead reads) does not fit a 32-bit index: the library must pick 64-bit cell
+    indices.  28 x 8190 x 8190 fp32 grid (padded 30 x 8192^2 = 2.013e9 cells, + 3 planes of 6.7e7 > 2^31), sources
+    next to the +z face so that most rays leave through it."""
+    if torch.cuda.mem_get_info()[1] < 150e9:
+        pytest.skip("needs the B200's memory")
+    nz, ny, nx = 28, 8190, 8190
+    pcell = (nz + 2) * (ny + 2) * (nx + 2)
+    assert pcell < 2 ** 31 <= pcell + 3 * (ny + 2) * (nx + 2)
+    g = torch.Generator(device="cuda").manual_seed(65)
+    nH = (torch.rand((nz, ny, nx), generator=g, device="cuda", dtype=torch.float32) + 0.5) * 1e-3
+    xHI = torch.rand((nz, ny, nx), generator=g, device="cuda", dtype=torch.float32) * 0.8 + 0.2
+    cfg = dict(name="guard64", n=None, shape=(nz, ny, nx), dx_cm=1.3e20, nH=nH, xHI=xHI,
+               src_pos=torch.tensor([[8188.5, 8187.5, 27.5], [4000.2, 4100.7, 26.1], [3.5, 8189.5, 27.9]], dtype=torch.float64),
+               src_L=torch.tensor([1e50, 3e50, 5e50], dtype=torch.float64),
+               params=synth.default_params(n_th=6e-4, e_excess_erg=1e-11))
+    gam, heat, sg, cg = _trace(cfg, cfg["src_pos"].numpy(), cfg["src_L"].numpy(), batch_rays=2 ** 20)
+    go, ho, so, co = run_oracle(O, cfg)
+    assert np.array_equal(cg[0], co[0]) and np.array_equal(cg[1], co[1])
+    for name in COUNTERS:
+        assert list(getattr(sg, name)) == list(getattr(so, name)), name
+    assert sg.segments == so.segments and sg.zero_len_segments == so.zero_len_segments
+    assert sg.neighbour_deposits == so.neighbour_deposits and sum(sg.exited) > 0
+    worst = compare_slabs(gam, heat, go, ho, cfg, slab=4)
+    assert float(gam[-1, -1, -1]) > 0.0
+    assert_budget(sg, "gpu")
+    print("guard-band 64-bit path: %d segments, %d rays left the box, worst relative Gamma error %.2e"
+          % (sg.segments, sum(sg.exited), worst))
