@@ -22,11 +22,15 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 ALGO_BYTES_PER_SEGMENT = {"f32": 48, "f64": 64}     # 4 field loads + 2 accumulator RMWs
+# the same without the assumption that every segment touches its neighbour: per segment 2 field loads + 1 RMW of the
+# cell, and the same again for each neighbour deposit the library counted (stats.neighbour_deposits)
+ALGO_BYTES_CELL = {"f32": 24, "f64": 32}
 METRIC = "ray_cell_segments_per_s"
-# Secondary (ALU / issue) roof of the march kernel: one ray-cell costs 230 executed warp
+# Secondary (issue) roof of the march kernel: one ray-cell costs 230 executed warp
 # instructions of which 76 are fp64 (profiles/r1_v12_march_config5.md); an fp64 warp instruction holds the
-# sub-partition's fp64 pipe for two cycles, so a warp-cell takes >= 230 + 76 issue cycles.
-ISSUE_CYCLES_PER_WARP_CELL = 306
+# sub-partition's fp64 pipe for two cycles while other instructions issue, so a warp-cell takes
+# max(230 issue slots, 2 x 76 fp64-pipe cycles) = 230 cycles of a scheduler.
+ISSUE_CYCLES_PER_WARP_CELL = 230
 SM_COUNT, SCHEDULERS_PER_SM, LANES = 148, 4, 32
 
 
@@ -40,7 +44,9 @@ def parse():
     ap.add_argument("--n-src", type=int, default=0, help="use only the first N sources (0 = all)")
     ap.add_argument("--batch-rays", type=int, default=0)
     ap.add_argument("--shard", action="store_true",
-                    help="N > 1: shard the step by source (one all-reduce of the photon grid) instead of N replicas")
+                    help="shard the step by source (one all-reduce of the photon grid); the default when N > 1")
+    ap.add_argument("--replicas", action="store_true",
+                    help="N > 1: every rank runs the whole step on its own GPU (no sharding, redundant work)")
     ap.add_argument("--spectrum-teff", type=float, default=0.0,
                     help="trace with the tau_0 lookup table of a black body of this temperature [K] (default: monochromatic)")
     ap.add_argument("--timestep-myr", type=float, default=0.0,
@@ -142,31 +148,51 @@ def make_workload(args, device):
     return cfg, pos, L
 
 
-def oracle_sample(cfg, pos, L, budget_s):
-    """The CPU oracle, as it stands, on a bounded sample of the same workload: the whole step (dedup,
-    merge, trace) on successive chunks of the source list until ~budget_s of CPU time is spent."""
+def cpu_info():
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    return model, os.cpu_count() or 1
+
+
+def oracle_sample(cfg, pos, L, budget_s, n_proc=0):
+    """The CPU oracle, as it stands, on a bounded sample of the same workload: the whole step (dedup, merge, ray
+    loop) on the first sources of the list, the ray loop spread over the host's cores (one single-threaded oracle
+    process per core over disjoint chunks of the sorted catalogue, oracle.step_parallel); the sample grows until one
+    run takes about budget_s seconds of wall time."""
     from oracle import oracle as O
-    import numpy as np
+    import psutil
     nH = cfg["nH"].cpu().numpy()
     xHI = cfg["xHI"].cpu().numpy()
     g = O.make_grid(cfg["shape"], cfg["dx_cm"], field_dtype=nH.dtype)
     p = O.make_params(**cfg["params"])
-    seg, t_used, n_used, chunk, a = 0, 0.0, 0, 8, 0
-    while t_used < budget_s and a < len(L):
-        b = min(len(L), a + chunk)
+    model, cores = cpu_info()
+    grid_bytes = nH.size * 8
+    n_proc = n_proc or max(1, min(cores, int(0.8 * psutil.virtual_memory().available // (grid_bytes + 2 ** 28))))
+    n, best = min(len(L), 4 * n_proc), None
+    while True:
         t0 = time.perf_counter()
-        _, _, st, _ = O.step(g, p, nH, xHI, pos[a:b], L[a:b], want_heat=True)
+        osum, cat = O.step_parallel(g, p, nH, xHI, pos[:n], L[:n], n_proc, want_heat=False, chunk=1)
         dt = time.perf_counter() - t0
-        seg += st.segments
-        t_used += dt
-        n_used += b - a
-        a = b
-        if dt < 0.2 * budget_s:
-            chunk = min(chunk * 2, 4096)
-    return dict(value=seg / t_used if t_used > 0 else 0.0, unit="segments/s", cores=1, kind="oracle",
-                sample="oracle.step (dedup, merge, trace, finalise) on the first %d of %d input sources of the same "
-                       "fields: %d segments in %.1f s, single thread" % (n_used, len(L), seg, t_used),
-                segments=int(seg), seconds=t_used)
+        seg, cpu_s = int(osum.stats.segments), osum.cpu_seconds
+        osum.close()
+        best = (seg, dt, cpu_s, n)
+        if dt >= 0.5 * budget_s or n >= len(L):
+            break
+        n = min(len(L), int(n * max(2.0, min(8.0, 0.8 * budget_s / max(dt, 1e-3)))))
+    seg, dt, cpu_s, n = best
+    return dict(value=seg / dt if dt > 0 else 0.0, unit="segments/s", cores=n_proc, kind="oracle",
+                cpu_model=model, host_cores=cores, per_core=seg / cpu_s if cpu_s > 0 else 0.0,
+                sample="oracle step (dedup, merge, ray loop; no heating grid) on the first %d of %d input sources of the "
+                       "same fields, ray loop on %d single-threaded processes: %d segments in %.1f s wall "
+                       "(%.3g segments/s per core)" % (n, len(L), n_proc, seg, dt, seg / max(cpu_s, 1e-9)),
+                segments=int(seg), seconds=dt)
 
 
 def run_reference(args):
@@ -190,7 +216,8 @@ def run_reference(args):
                warmup=args.warmup, ms_per_step=1e3 * sec / args.steps, higher_is_better=True, scaling="weak",
                vs_baseline=None, dtype="f64", data="synthetic",
                config=dict(workload=cfg["name"], notes=cfg["notes"], sample=last["sample"]),
-               cpu_baseline=dict(value=v, unit="segments/s", cores=1, kind="oracle", sample=last["sample"]),
+               cpu_baseline=dict(value=v, unit="segments/s", cores=last["cores"], kind="oracle", sample=last["sample"],
+                                 cpu_model=last["cpu_model"], host_cores=last["host_cores"]),
                e2e=dict(value=v, unit="segments/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0))
     print(json.dumps(out))
 
@@ -212,6 +239,8 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if not args.replicas:
+            args.shard = True                  # N ranks divide the step's sources (real work, counted once)
 
     def barrier():
         if world > 1:
@@ -273,6 +302,7 @@ def main():
         clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     seg = 0
+    nbr = 0
     ms_march = 0.0
     launches = 0
     march_launches = 0
@@ -281,6 +311,7 @@ def main():
     for _ in range(args.steps):
         st = step()
         seg += st.segments
+        nbr += st.neighbour_deposits
         ms_march += st.ms_march
         launches += st.kernel_launches + 3            # + prep_fields, sum_partials, snap
         march_launches += st.march_launches
@@ -332,6 +363,13 @@ def main():
                     peak_source=peak_src,
                     note="achieved = %d B x segments / sum of march-launch durations (CUDA events around every "
                          "launch on the launching stream); DRAM traffic per launch: see profiles/" % bps)
+        # the same with the neighbour traffic counted, not assumed: (2 field loads + 1 accumulator RMW) per segment
+        # and per neighbour deposit the library counted
+        cb = ALGO_BYTES_CELL[fdt]
+        ach_x = cb * (seg + nbr) / (ms_march * 1e-3) / 1e9
+        roof["counted"] = dict(achieved=ach_x, frac=ach_x / peak, bytes_per_segment=cb * (seg + nbr) / max(seg, 1),
+                               neighbour_deposits_per_segment=nbr / max(seg, 1),
+                               note="%d B per segment + %d B per counted neighbour deposit" % (cb, cb))
         sm_hz = 1e6 * float((clk or {}).get("sm_mhz") or 1965.0)
         alu_peak = SM_COUNT * SCHEDULERS_PER_SM * sm_hz * LANES / ISSUE_CYCLES_PER_WARP_CELL
         roof["alu"] = dict(bound="alu", achieved=seg / (ms_march * 1e-3), peak=alu_peak, unit="segments/s",
@@ -339,16 +377,25 @@ def main():
                            note="issue-slot roof of the march kernel: SMs x 4 schedulers x SM clock x 32 lanes / %d issue "
                                 "cycles per warp-cell (all lanes busy, no stall); the kernel is bound by this, not by HBM"
                                 % ISSUE_CYCLES_PER_WARP_CELL)
-        tfile = os.path.join(ROOT, "profiles", "march_traffic.csv")     # measured by ncu, see profiles/*.md
-        if os.path.exists(tfile):
+        # DRAM bytes per march launch measured by ncu on THIS workload (profiles/march_traffic.csv, one row per
+        # captured launch; profiles/march_traffic.md has the commands); null when no capture matches the run
+        tfile = os.path.join(ROOT, "profiles", "march_traffic.csv")
+        roof["traffic_note"] = "no ncu capture of this workload in profiles/march_traffic.csv"
+        if os.path.exists(tfile) and not args.shard and args.timestep_myr == 0:
             try:
                 import csv
                 with open(tfile, newline="") as f:
-                    for row in csv.DictReader(f):
-                        if row.get("dram_bytes_per_launch"):
-                            roof["traffic"] = float(row["dram_bytes_per_launch"])
-                            break
-            except (ValueError, OSError):
+                    rows = [r for r in csv.DictReader(f)
+                            if r.get("workload") == cfg["name"] and int(r.get("n_sources", -1)) == len(L)
+                            and int(r.get("periodic", -1)) == int(args.periodic)
+                            and r.get("spectrum") == ("table" if args.spectrum_teff > 0 else "monochromatic")]
+                if rows:
+                    tb = [1e9 * (float(r["dram_read_gb"]) + float(r["dram_write_gb"])) for r in rows]
+                    tm = [float(r["launch_ms"]) for r in rows]
+                    roof["traffic"] = sum(tb) / len(tb)
+                    roof["traffic_note"] = ("mean dram__bytes_read.sum + dram__bytes_write.sum of %d captured march launches "
+                                            "of this workload (ncu --set full, mean %.2f ms under ncu)" % (len(tb), sum(tm) / len(tm)))
+            except (ValueError, OSError, KeyError):
                 pass
         cpu = None
         if not args.no_cpu:

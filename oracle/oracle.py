@@ -336,3 +336,103 @@ def blackbody_table(t_eff_K, e_lo, e_hi, m):
     _chk(lib().orc_blackbody_table(C.c_double(t_eff_K), C.c_int(e_lo), C.c_int(e_hi), C.c_int(m), _ptr(q), C.c_int64(n)),
          "blackbody_table")
     return q
+
+
+# ---- the step on P host cores (SURVEY.md 8(d) "Oracle timed beside it") ---------------------------------------------
+# Gamma is a sum over sources: the parent runs the source pass once (dedup, radii, merge, sort), P
+# single-threaded worker processes then trace disjoint chunks of the sorted catalogue with the unchanged
+# orc_trace loop (orc_trace_add), each adding into its own grids (shared memory, zero-filled by the OS), and the
+# parent adds the counters; the grids are added by the caller, slab by slab.  Process management only.
+
+def _worker(g, p, nH, xHI, cat, chunks, counter, shm_names, shape, want_heat, conn):
+    import time
+    from multiprocessing import shared_memory
+    shms = [shared_memory.SharedMemory(name=n) for n in shm_names]
+    gam = np.ndarray(shape, np.float64, buffer=shms[0].buf)
+    heat = np.ndarray(shape, np.float64, buffer=shms[1].buf) if want_heat else None
+    st = Stats()
+    t0 = time.perf_counter()
+    while True:
+        with counter.get_lock():
+            k = counter.value
+            counter.value += 1
+        if k >= len(chunks):
+            break
+        a, b = chunks[k]
+        trace_add(g, p, nH, xHI, cat[0][a:b], cat[1][a:b], gam, heat, st)
+    conn.send((bytes(st), time.perf_counter() - t0))
+    conn.close()
+    del gam, heat
+    for s in shms:
+        s.close()
+
+
+class OracleSum:
+    """Partial results of the worker processes: the summed counters (a Stats) and the partial grids;
+    gamma(z0, z1) / heat(z0, z1) add the partial grids of a z-slab."""
+
+    def __init__(self, stats, gam_parts, heat_parts, shms, cpu_seconds, n_proc):
+        self.stats, self._g, self._h, self._shms = stats, gam_parts, heat_parts, shms
+        self.cpu_seconds, self.n_proc = cpu_seconds, n_proc
+
+    def gamma(self, z0=0, z1=None):
+        return np.sum([g[z0:z1] for g in self._g], axis=0)
+
+    def heat(self, z0=0, z1=None):
+        return np.sum([h[z0:z1] for h in self._h], axis=0) if self._h else None
+
+    def close(self):
+        self._g = self._h = None
+        for s in self._shms:
+            s.close()
+            s.unlink()
+        self._shms = []
+
+
+def step_parallel(g, p, nH, xHI, pos, L, n_proc, want_heat=True, chunk=4):
+    """The whole RT step with the ray loop on n_proc processes.  Returns (OracleSum, catalogue); the caller must
+    close() the OracleSum."""
+    import multiprocessing as mp
+    from multiprocessing import shared_memory
+    nH = _field(g, nH)
+    xHI = _field(g, xHI)
+    st0, cat = catalogue(g, p, xHI, pos, L)
+    n_cat = len(cat[1])
+    chunks = [(a, min(n_cat, a + chunk)) for a in range(0, n_cat, chunk)]
+    shape = (g.nz, g.ny, g.nx)
+    nbytes = int(np.prod(shape)) * 8
+    ctx = mp.get_context("fork")
+    counter = ctx.Value(C.c_int64, 0)
+    shms, procs, conns, gam_parts, heat_parts = [], [], [], [], []
+    for _ in range(n_proc):
+        pair = [shared_memory.SharedMemory(create=True, size=nbytes) for _ in range(2 if want_heat else 1)]
+        shms += pair
+        gam_parts.append(np.ndarray(shape, np.float64, buffer=pair[0].buf))
+        if want_heat:
+            heat_parts.append(np.ndarray(shape, np.float64, buffer=pair[1].buf))
+        rx, tx = ctx.Pipe(duplex=False)
+        pr = ctx.Process(target=_worker, args=(g, p, nH, xHI, cat, chunks, counter, [s.name for s in pair], shape,
+                                               want_heat, tx))
+        pr.start()
+        tx.close()
+        procs.append(pr)
+        conns.append(rx)
+    total = Stats()
+    cpu = 0.0
+    for pr, rx in zip(procs, conns):
+        raw, secs = rx.recv()
+        pr.join()
+        if pr.exitcode != 0:
+            raise RuntimeError("oracle worker failed")
+        st = Stats.from_buffer_copy(raw)
+        cpu += secs
+        for name, _ in Stats._fields_:
+            v = getattr(st, name)
+            if hasattr(v, "__len__"):
+                t = getattr(total, name)
+                for l in range(len(v)):
+                    t[l] += v[l]
+            else:
+                setattr(total, name, getattr(total, name) + v)
+    total.n_src_in, total.n_src_dedup, total.n_src_merged = st0.n_src_in, st0.n_src_dedup, st0.n_src_merged
+    return OracleSum(total, gam_parts, heat_parts, shms, cpu, n_proc), cat

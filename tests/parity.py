@@ -120,108 +120,15 @@ def compare_slabs(gam_gpu, heat_gpu, go, ho, cfg, params=None, slab=32):
     return worst
 
 
-# ---- the oracle on P host cores (SURVEY.md 8(d) "Oracle timed beside it") -------------------------------------------
-# Gamma is a sum over sources: the parent runs the source pass once (dedup, radii, merge, sort), P
-# single-threaded worker processes then trace disjoint chunks of the sorted catalogue with the unchanged
-# orc_trace loop, each adding into its own grids (shared memory), and the parent adds the P grids and the counters.
-
-def _oracle_worker(rank, g, p, nH, xHI, cat, chunks, counter, shm_names, shape, want_heat, conn):
-    from multiprocessing import shared_memory
-    from oracle import oracle as O
-    import time
-    shms = [shared_memory.SharedMemory(name=n) for n in shm_names]
-    gam = np.ndarray(shape, np.float64, buffer=shms[0].buf)
-    heat = np.ndarray(shape, np.float64, buffer=shms[1].buf) if want_heat else None
-    st = O.Stats()
-    t0 = time.perf_counter()
-    while True:
-        with counter.get_lock():
-            k = counter.value
-            counter.value += 1
-        if k >= len(chunks):
-            break
-        a, b = chunks[k]
-        O.trace_add(g, p, nH, xHI, cat[0][a:b], cat[1][a:b], gam, heat, st)
-    conn.send((bytes(st), time.perf_counter() - t0))
-    conn.close()
-    del gam, heat
-    for s in shms:
-        s.close()
-
-
-class OracleSum:
-    """Partial results of the worker processes: summed counters (shaped like the oracle's Stats) and the list of
-    partial grids; `gamma(z0, z1)` / `heat(z0, z1)` add the partial grids of a z-slab."""
-
-    def __init__(self, stats, gam_parts, heat_parts, shms, cpu_seconds, n_proc):
-        self.stats, self._g, self._h, self._shms = stats, gam_parts, heat_parts, shms
-        self.cpu_seconds, self.n_proc = cpu_seconds, n_proc
-
-    def gamma(self, z0=0, z1=None):
-        return np.sum([g[z0:z1] for g in self._g], axis=0)
-
-    def heat(self, z0=0, z1=None):
-        return np.sum([h[z0:z1] for h in self._h], axis=0) if self._h else None
-
-    def close(self):
-        self._g = self._h = None
-        for s in self._shms:
-            s.close()
-            s.unlink()
-        self._shms = []
-
+# ---- the oracle on P host cores (SURVEY.md 8(d) "Oracle timed beside it"): oracle/oracle.py step_parallel ---------------
 
 def run_oracle_parallel(O, cfg, n_proc, params=None, periodic=0, want_heat=True, chunk=4):
     """Returns (OracleSum, catalogue).  The caller must close() the OracleSum (shared memory)."""
-    import ctypes
-    import multiprocessing as mp
-    from multiprocessing import shared_memory
     p = dict(cfg["params"])
     p.update(params or {})
     nH, xHI, pos, L = oracle_inputs(cfg)
     g = O.make_grid(cfg["shape"], cfg["dx_cm"], field_dtype=nH.dtype, periodic=periodic)
-    pp = O.make_params(**p)
-    st0, cat = O.catalogue(g, pp, xHI, pos, L)
-    n_cat = len(cat[1])
-    chunks = [(a, min(n_cat, a + chunk)) for a in range(0, n_cat, chunk)]
-    shape = tuple(cfg["shape"])
-    nbytes = int(np.prod(shape)) * 8
-    ctx = mp.get_context("fork")
-    counter = ctx.Value(ctypes.c_int64, 0)
-    shms, procs, conns, gam_parts, heat_parts = [], [], [], [], []
-    for r in range(n_proc):
-        pair = [shared_memory.SharedMemory(create=True, size=nbytes) for _ in range(2 if want_heat else 1)]
-        shms += pair
-        gam_parts.append(np.ndarray(shape, np.float64, buffer=pair[0].buf))
-        gam_parts[-1][...] = 0.0
-        if want_heat:
-            heat_parts.append(np.ndarray(shape, np.float64, buffer=pair[1].buf))
-            heat_parts[-1][...] = 0.0
-        rx, tx = ctx.Pipe(duplex=False)
-        pr = ctx.Process(target=_oracle_worker, args=(r, g, pp, nH, xHI, cat, chunks, counter, [s.name for s in pair],
-                                                      shape, want_heat, tx))
-        pr.start()
-        tx.close()
-        procs.append(pr)
-        conns.append(rx)
-    total = O.Stats()
-    cpu = 0.0
-    for pr, rx in zip(procs, conns):
-        raw, secs = rx.recv()
-        pr.join()
-        assert pr.exitcode == 0
-        st = O.Stats.from_buffer_copy(raw)
-        cpu += secs
-        for name, _ in O.Stats._fields_:
-            v = getattr(st, name)
-            if hasattr(v, "__len__"):
-                t = getattr(total, name)
-                for l in range(len(v)):
-                    t[l] += v[l]
-            else:
-                setattr(total, name, getattr(total, name) + v)
-    total.n_src_in, total.n_src_dedup, total.n_src_merged = st0.n_src_in, st0.n_src_dedup, st0.n_src_merged
-    return OracleSum(total, gam_parts, heat_parts, shms, cpu, n_proc), cat
+    return O.step_parallel(g, O.make_params(**p), nH, xHI, pos, L, n_proc, want_heat=want_heat, chunk=chunk)
 
 
 def compare_slabs_sum(gam_gpu, heat_gpu, osum, cfg, params=None, slab=32):
