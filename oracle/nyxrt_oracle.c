@@ -412,7 +412,7 @@ int orc_merge(const orc_grid *g, const orc_params *p, int64_t n, const int32_t *
 /* binary representation of tau_0 (R38): 2^m nodes per octave, linear in tau_0 inside an octave,    */
 /* from 2^e_lo to 2^e_hi; linear from 0 below 2^e_lo; constant above 2^e_hi.                        */
 
-static struct { int on, e_lo, e_hi, m; int64_t n; double *q; } g_lut;
+static struct { int on, e_lo, e_hi, m; int64_t n; double *q; double *t; double tau_thin; } g_lut;
 
 int64_t orc_spectrum_nodes(int e_lo, int e_hi, int m) { return (((int64_t)(e_hi - e_lo)) << m) + 1; }
 
@@ -424,6 +424,7 @@ double orc_spectrum_node_tau(int e_lo, int m, int64_t k) {
 
 int orc_set_spectrum(int e_lo, int e_hi, int m, const double *q, int64_t n) {
     free(g_lut.q);
+    free(g_lut.t);
     memset(&g_lut, 0, sizeof g_lut);
     if (!q) return ORC_OK;                                              /* back to monochromatic */
     if (e_lo < -1000 || e_hi > 1000 || e_hi <= e_lo || m < 0 || m > 20 || n != orc_spectrum_nodes(e_lo, e_hi, m))
@@ -448,11 +449,49 @@ double orc_spectrum_q(double tau) {
     return fma(frac, g_lut.q[k + 1] - g_lut.q[k], g_lut.q[k]);
 }
 
-/* absorbed fraction of a ray's share between the source and optical depth tau; photons absorbed in a
+/* S4: the separate table for the optically thin case (PAPER.md:267 footnote 3: "the approach of C2-Ray, which
+   takes the limit as n_H -> 0 to compute a separate LUT for the optically thin case"; with PAPER.md:95).  In the
+   limit of a thin cell Eq. 1's factor (1 - exp(-dtau_nu)) -> dtau_nu = dtau_0 (nu/nu_0)^-3, so the share absorbed in
+   the cell is dtau_0 T(tau_0) with
+       T(tau_0) = int phi(nu) (nu/nu_0)^-3 exp(-tau_0 (nu/nu_0)^-3) dnu  =  dQ/dtau_0,
+   tabulated on the nodes of Q and interpolated the same way (constant below the first node and above the last)
+   [R40].  A segment with dtau_0 < tau_thin takes dtau_0 T(tau_0 + dtau_0 / 2) instead of Q(tau_0 + dtau_0) -
+   Q(tau_0), the difference of two interpolants that cancels there [R41].  The two forms do not telescope into
+   each other, so with the thin table set the photons a ray carries are counted down segment by segment instead of
+   being read off Q(tau_0) [R42].  The neighbour's share (Eq. 6 / 8) is (1 - f_c) of whatever the segment absorbed,
+   in photons: no quotient of absorber densities is formed, which is the part the footnote calls "not applicable". */
+int orc_set_spectrum_thin(const double *t, int64_t n, double tau_thin) {
+    free(g_lut.t);
+    g_lut.t = NULL;
+    g_lut.tau_thin = 0.0;
+    if (!t) return ORC_OK;
+    if (!g_lut.on || n != g_lut.n || !(tau_thin >= 0.0)) return ORC_EINVAL;
+    g_lut.t = malloc((size_t)n * sizeof *t);
+    if (!g_lut.t) return ORC_ENOMEM;
+    memcpy(g_lut.t, t, (size_t)n * sizeof *t);
+    g_lut.tau_thin = tau_thin;
+    return ORC_OK;
+}
+
+double orc_spectrum_t(double tau) {
+    if (!(tau >= ldexp(1.0, g_lut.e_lo))) return g_lut.t[0];
+    if (tau >= ldexp(1.0, g_lut.e_hi)) return g_lut.t[g_lut.n - 1];
+    uint64_t bits;
+    memcpy(&bits, &tau, sizeof bits);
+    const int fb = 52 - g_lut.m;
+    int64_t k = (int64_t)(bits >> fb) - ((int64_t)(g_lut.e_lo + 1023) << g_lut.m);
+    double frac = ldexp((double)(bits & (((uint64_t)1 << fb) - 1)), -fb);
+    return fma(frac, g_lut.t[k + 1] - g_lut.t[k], g_lut.t[k]);
+}
+
+/* absorbed fraction of a ray's share between the source and optical depth tau; share absorbed in a
    segment from tau to tau + dtau (Eq. 1 with V_box) */
 static double remaining_at(double tau) { return g_lut.on ? 1.0 - orc_spectrum_q(tau) : exp(-tau); }
 static double absorbed_in(double tau, double dtau) {
-    if (g_lut.on) return orc_spectrum_q(tau + dtau) - orc_spectrum_q(tau);
+    if (g_lut.on) {
+        if (g_lut.t && dtau < g_lut.tau_thin) return dtau * orc_spectrum_t(tau + 0.5 * dtau);     /* R41 */
+        return orc_spectrum_q(tau + dtau) - orc_spectrum_q(tau);
+    }
     return exp(-tau) * (-expm1(-dtau));
 }
 
@@ -468,7 +507,8 @@ static double bb_integral(double x0, double tau, int with_abs) {
         double x = x0 + u / (1.0 - u);
         double jac = 1.0 / ((1.0 - u) * (1.0 - u));
         double f = x * x / expm1(x) * jac;
-        if (with_abs) { double r = x0 / x; f *= -expm1(-tau * r * r * r); }
+        if (with_abs == 1) { double r = x0 / x; f *= -expm1(-tau * r * r * r); }
+        if (with_abs == 2) { double r = x0 / x; f *= (r * r * r) * exp(-tau * r * r * r); }    /* thin table T */
         double wgt = (i == 0) ? 1.0 : ((i & 1) ? 4.0 : 2.0);
         sum += wgt * f;
     }
@@ -480,6 +520,15 @@ int orc_blackbody_table(double t_eff_K, int e_lo, int e_hi, int m, double *q, in
     const double x0 = 13.598434 * 1.602176634e-19 / (1.380649e-23 * t_eff_K);   /* h nu_0 / k T */
     const double norm = bb_integral(x0, 0.0, 0);
     for (int64_t k = 0; k < n; ++k) q[k] = bb_integral(x0, orc_spectrum_node_tau(e_lo, m, k), 1) / norm;
+    return ORC_OK;
+}
+
+/* T = dQ/dtau_0 of the same black body on the same nodes (S4, R40) */
+int orc_blackbody_thin_table(double t_eff_K, int e_lo, int e_hi, int m, double *t, int64_t n) {
+    if (!(t_eff_K > 0.0) || n != orc_spectrum_nodes(e_lo, e_hi, m)) return ORC_EINVAL;
+    const double x0 = 13.598434 * 1.602176634e-19 / (1.380649e-23 * t_eff_K);
+    const double norm = bb_integral(x0, 0.0, 0);
+    for (int64_t k = 0; k < n; ++k) t[k] = bb_integral(x0, orc_spectrum_node_tau(e_lo, m, k), 2) / norm;
     return ORC_OK;
 }
 
@@ -500,11 +549,14 @@ typedef struct {
     double L_src;
 } tracer;
 
-static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
+/* carried: photons/s the ray holds at birth; used (and counted down) only when the thin table is set (R42) */
+static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau, double carried) {
     const orc_grid *g = T->g;
     const orc_params *p = T->p;
     orc_stats *st = T->st;
     const double L_ray = T->L_src / (12.0 * ldexp(1.0, 2 * level));   /* L shared evenly */
+    const int count_down = g_lut.on && g_lut.t != NULL;
+#define RAY_PHOTONS() (count_down ? carried : L_ray * remaining_at(tau))
     double d[3], inv[3], sx[3];
     int64_t o[3];
     orc_pix2dir(level, pix, d);
@@ -523,33 +575,33 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
     }
     if (!g->periodic && !in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
         st->exited[level]++;
-        T->escaped += (long double)(L_ray * remaining_at(tau));
+        T->escaped += (long double)RAY_PHOTONS();
         return;
     }
     for (;;) {
         /* 1. kill (RAY_FLTR tau test; per cell, R14) */
         if (tau >= p->tau_max) {
             st->killed_tau[level]++;
-            T->residual += (long double)(L_ray * remaining_at(tau));
+            T->residual += (long double)RAY_PHOTONS();
             return;
         }
         /* 2. l_max */
         if (level >= p->level_max) {
             st->killed_lmax[level]++;
-            T->residual += (long double)(L_ray * remaining_at(tau));
+            T->residual += (long double)RAY_PHOTONS();
             return;
         }
         /* 2b. periodic box: the ray ends once its travel distance is no longer below sqrt(3) L_box
            (RAY_FLTR); counted with the rays that left the system (reading R30) */
         if (g->periodic && !(s < T->s_max)) {
             st->exited[level]++;
-            T->escaped += (long double)(L_ray * remaining_at(tau));
+            T->escaped += (long double)RAY_PHOTONS();
             return;
         }
         /* 3. split, Eq. 4: Omega_c/Omega(l) < N_min  <=>  s^2 > 3 4^l/(pi N_min) */
         if (s * s > T->r2_split[level]) {
             st->split[level]++;
-            for (int k = 0; k < 4; ++k) trace_ray(T, level + 1, 4 * pix + k, s, tau);
+            for (int k = 0; k < 4; ++k) trace_ray(T, level + 1, 4 * pix + k, s, tau, 0.25 * carried);
             return;
         }
         /* 4. one cell (Amanatides-Woo, PAPER.md:152 [76]) */
@@ -639,6 +691,7 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
                 T->log_n++;
             }
             tau = tau + dtau;
+            carried = carried - dN;
         } else {
             st->zero_len_segments++;
         }
@@ -647,11 +700,12 @@ static void trace_ray(tracer *T, int level, int64_t pix, double s, double tau) {
         sx[ax] = ((double)(o[ax] + (d[ax] > 0.0 ? 1 : 0)) - 0.5) * inv[ax];
         if (!g->periodic && !in_box(g, T->src_cell[0] + o[0], T->src_cell[1] + o[1], T->src_cell[2] + o[2])) {
             st->exited[level]++;                                        /* R20 */
-            T->escaped += (long double)(L_ray * remaining_at(tau));
+            T->escaped += (long double)RAY_PHOTONS();
             return;
         }
     }
 }
+#undef RAY_PHOTONS
 
 /* gamma, heat: [nz][ny][nx] double; heat may be NULL.  zero != 0: overwritten; zero == 0: the deposits are ADDED
    to what the grids hold and the counters to *st (Gamma is a sum over sources: a catalogue can be
@@ -686,7 +740,7 @@ static int trace_catalogue(const orc_grid *g, const orc_params *p, const void *n
         T.src_id = (int32_t)a;
         T.L_src = L[a];
         emitted += (long double)L[a];
-        for (int64_t pix = 0; pix < 12; ++pix) trace_ray(&T, 0, pix, 0.0, 0.0);   /* PAPER.md:111 */
+        for (int64_t pix = 0; pix < 12; ++pix) trace_ray(&T, 0, pix, 0.0, 0.0, L[a] / 12.0);   /* PAPER.md:111 */
     }
     if (zero) {
         st->photons_emitted = (double)emitted;

@@ -324,6 +324,30 @@ def set_spectrum(e_lo=0, e_hi=0, m=0, q=None):
     _chk(lib().orc_set_spectrum(C.c_int(e_lo), C.c_int(e_hi), C.c_int(m), _ptr(q), C.c_int64(len(q))), "set_spectrum")
 
 
+def set_spectrum_thin(t=None, tau_thin=0.0):
+    """The separate table for thin segments (PAPER.md:267 footnote 3), on the nodes of the table set with
+    set_spectrum; t = None: off."""
+    if t is None:
+        _chk(lib().orc_set_spectrum_thin(None, C.c_int64(0), C.c_double(0.0)), "set_spectrum_thin")
+        return
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    _chk(lib().orc_set_spectrum_thin(_ptr(t), C.c_int64(len(t)), C.c_double(tau_thin)), "set_spectrum_thin")
+
+
+def spectrum_t(tau):
+    f = lib().orc_spectrum_t
+    f.restype = C.c_double
+    return f(C.c_double(tau))
+
+
+def blackbody_thin_table(t_eff_K, e_lo, e_hi, m):
+    n = spectrum_nodes(e_lo, e_hi, m)
+    t = np.zeros(n)
+    _chk(lib().orc_blackbody_thin_table(C.c_double(t_eff_K), C.c_int(e_lo), C.c_int(e_hi), C.c_int(m), _ptr(t),
+                                        C.c_int64(n)), "blackbody_thin_table")
+    return t
+
+
 def spectrum_q(tau):
     f = lib().orc_spectrum_q
     f.restype = C.c_double
