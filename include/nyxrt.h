@@ -163,6 +163,20 @@ int nyxrt_spectrum_node_tau(int32_t e_lo, int32_t m, int64_t k, double *tau);
 int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, const double *h_q, int64_t n);
 int nyxrt_blackbody_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_q, int64_t n);
 
+/* The separate table for the optically thin case (PAPER.md:267 footnote 3: "the approach of C2-Ray, which takes the
+ * limit as n_H -> 0 to compute a separate LUT for the optically thin case"; readings R40-R42).  In a thin cell Eq. 1's
+ * (1 - exp(-dtau_nu)) -> dtau_nu, so the cell absorbs share * dtau_0 * T(tau_0) with
+ *     T(tau_0) = int phi(nu) (nu/nu_0)^-3 exp(-tau_0 (nu/nu_0)^-3) dnu = dQ/dtau_0,
+ * on the nodes of the Q table set before (same n), linear between nodes, constant below the first and above the last.
+ * A segment with dtau_0 < tau_thin absorbs share * dtau_0 * T(tau_0 + dtau_0 / 2) instead of the difference of two
+ * interpolated Q values; the photons a ray carries are then counted down segment by segment (the two forms do not
+ * telescope into each other).  The neighbour's share of Eq. 6 / 8 is (1 - f_c) of the absorbed photons either way.
+ *   nyxrt_set_spectrum_thin    h_t: host array of n values >= 0, copied (h_t = NULL: thin table off).  A later
+ *                              nyxrt_set_spectrum drops it.  Errors: EINVAL, ESTATE (no Q table), ECUDA.
+ *   nyxrt_blackbody_thin_table T of a black body of temperature t_eff_K above 13.6 eV on the given nodes. */
+int nyxrt_set_spectrum_thin(nyxrt_ctx *ctx, const double *h_t, int64_t n, double tau_thin);
+int nyxrt_blackbody_thin_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_t, int64_t n);
+
 /* Source sharding across GPUs: Gamma is a sum over sources, so
  * each of `world` processes, holding a full replica of the fields and the full source list, traces the
  * catalogue entries rank, rank + world, ... (the catalogue -- dedup, merge, sort -- is computed by every

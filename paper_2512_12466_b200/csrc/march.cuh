@@ -158,11 +158,11 @@ struct OptArray { V v[N]; };
 template <typename V, int N>
 struct OptArray<false, V, N> {};          // not needed by this instantiation: takes no shared memory
 
-template <bool LUT>
+template <int LUT>
 struct ThreadScratch {
     unsigned long long key[MARCH_THREADS];
     double esc[MARCH_THREADS], res[MARCH_THREADS];
-    OptArray<LUT, double, MARCH_THREADS> w;   // spectrum table: the ray's share of its source's photons (constant)
+    OptArray<LUT != 0, double, MARCH_THREADS> w;   // spectrum table: the ray's share of its source's photons (constant)
     double d[3][MARCH_THREADS];          // the lane's ray: HEALPix direction and 1/d (read-only while it marches;
     double inv[3][MARCH_THREADS];        // kept out of the register file so that 5 blocks fit an SM)
 };
@@ -186,6 +186,18 @@ __device__ __forceinline__ double lut_q(const MarchArgs &A, double tau) {
     const double frac = (double)(bits & A.lut_fmask) * A.lut_fscale;
     const double q0 = __ldg(A.lut_q + k), q1 = __ldg(A.lut_q + k + 1);
     return fma(frac, q1 - q0, q0);
+}
+
+// The separate table for thin segments (PAPER.md:267 footnote 3; R40): T = dQ/dtau_0 on the nodes of Q, the same
+// interpolation, constant below the first node and above the last.
+__device__ __forceinline__ double lut_t(const MarchArgs &A, double tau) {
+    if (!(tau >= A.lut_t_lo)) return A.lut_t_first;
+    if (tau >= A.lut_t_hi) return A.lut_t_last;
+    const long long bits = __double_as_longlong(tau);
+    const long long k = (bits >> A.lut_fb) - A.lut_k0;
+    const double frac = (double)(bits & A.lut_fmask) * A.lut_fscale;
+    const double t0 = __ldg(A.lut_t + k), t1 = __ldg(A.lut_t + k + 1);
+    return fma(frac, t1 - t0, t0);
 }
 
 // One ray-cell segment, described by the geometry stage and consumed by the physics stage one iteration
@@ -221,9 +233,12 @@ constexpr unsigned long long WRAP_MASK = (1ull << WRAP_BITS) - 1ull;
 // GEOM: 0 no correction, 1 Eq. 5 only, 3 Eq. 5-6 / 7-8 (neighbour deposit; flags live in the field), 4 squared
 // PER: periodic box: cells wrap, rays end at s >= sqrt(3) L_box, the halo holds the wrapped
 // images of the opposite faces (neighbour reads) and deposits into it are folded back by finalise.
-// LUT: absorbed photons from the spectrum table, w [Q(tau + dtau) - Q(tau)], instead of the monochromatic
+// LUT = 2: the Q table plus the table for thin segments (R40-R42): a segment with dtau < tau_thin absorbs
+// w dtau T(tau + dtau / 2); N is the photon count the ray carries, counted down segment by segment, as in the
+// monochromatic kernel, and the share w is recomputed from the source's luminosity when the ray is popped.
+// LUT = 1: absorbed photons from the spectrum table, w [Q(tau + dtau) - Q(tau)], instead of the monochromatic
 // N (1 - e^-dtau); the lane's N register then holds Q(tau) and the pool's N the share w.
-template <int GEOM, typename IDX, bool PER, bool LUT>
+template <int GEOM, typename IDX, bool PER, int LUT>
 __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(const __grid_constant__ MarchArgs A) {
     __shared__ ThreadScratch<LUT> T;
     __shared__ RayQueue<IDX, PER> Q;
@@ -366,7 +381,13 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 ++n_seg;
                 const double dtau = (fabs(D.a_c) * sdx) * D.ds;
                 double pm, left, dN;
-                if constexpr (LUT) {
+                if constexpr (LUT == 2) {
+                    const double frac = dtau < A.tau_thin ? dtau * lut_t(A, tau + 0.5 * dtau)
+                                                           : lut_q(A, tau + dtau) - lut_q(A, tau);
+                    dN = T.w.v[threadIdx.x] * frac;
+                    left = N - dN;
+                    pm = 0.0;
+                } else if constexpr (LUT == 1) {
                     left = lut_q(A, tau + dtau);                                  // Q at the end of the segment
                     dN = T.w.v[threadIdx.x] * (left - N);
                 } else {
@@ -387,7 +408,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                     }
                     atomicAdd(acc + D.c, fc * dN);
                 }
-                N = LUT ? left : N * left;
+                N = LUT != 0 ? left : N * left;
                 tau = tau + dtau;
             } else {
                 ++n_zero;
@@ -520,7 +541,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
             qhead = 0;
             qn = __popc(m_park);
             __syncwarp();
-            retire(outcome, ts, ttau, (LUT && outcome != OUT_NONE) ? tN * (1.0 - lut_q(A, ttau)) : tN, tN, ikey);
+            retire(outcome, ts, ttau, (LUT == 1 && outcome != OUT_NONE) ? tN * (1.0 - lut_q(A, ttau)) : tN, tN, ikey);
             continue;
         }
         // ---- pop: idle lanes take parked rays ------------------------------------------------------------
@@ -533,7 +554,9 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 const int e = qhead + rank;
                 T.key[threadIdx.x] = Q.key[wid][e];
                 s = Q.s[wid][e]; tau = Q.tau[wid][e]; N = Q.N[wid][e];
-                if constexpr (LUT) { T.w.v[threadIdx.x] = N; N = lut_q(A, tau); }
+                if constexpr (LUT == 1) { T.w.v[threadIdx.x] = N; N = lut_q(A, tau); }
+                if constexpr (LUT == 2)                                           // the share L / (12 4^l)
+                    T.w.v[threadIdx.x] = A.cat_L[key_src(Q.key[wid][e])] / (12.0 * (double)(1ll << (2 * level)));
                 const double d0 = Q.d0[wid][e], d1 = Q.d1[wid][e], d2 = Q.d2[wid][e];
                 const double inv0 = Q.inv0[wid][e], inv1 = Q.inv1[wid][e], inv2 = Q.inv2[wid][e];
                 T.d[0][threadIdx.x] = d0; T.d[1][threadIdx.x] = d1; T.d[2][threadIdx.x] = d2;
@@ -583,7 +606,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 }
             }
         }
-        if constexpr (LUT) {
+        if constexpr (LUT == 1) {
             const double w = T.w.v[threadIdx.x];
             retire(outcome, s, tau, w * (1.0 - N), w, outcome == OUT_SPLIT ? T.key[threadIdx.x] : 0ull);
         } else {

@@ -73,6 +73,8 @@ struct nyxrt_ctx {
     int shard_rank, shard_world;           // source sharding (nyxrt_set_shard); 0 of 1 = everything
     double r2_split[MAXLEV], K[MAXLEV];
     double *d_lut;                         // spectrum table on the device (nyxrt_set_spectrum), or null
+    double *d_lut_t;                       // table for thin segments (nyxrt_set_spectrum_thin), or null
+    double lut_t_first, lut_t_last, tau_thin;
     int lut_e_lo, lut_e_hi, lut_m;
     long long lut_n;
     double lut_first, lut_last;
@@ -216,7 +218,7 @@ long long default_batch(const nyxrt_ctx *c) {
 
 constexpr size_t MARCH_SMEM = 0;          // the kernel's scratch is static shared memory
 
-template <int GEOM, bool LUT>
+template <int GEOM, int LUT>
 void launch_march(const MarchArgs &a, bool idx64, bool per, int blocks, cudaStream_t st) {
     if (per) {
         if (idx64) march_kernel<GEOM, long long, true, LUT><<<blocks, MARCH_THREADS, MARCH_SMEM, st>>>(a);
@@ -234,7 +236,7 @@ cudaError_t setup_kernel(K kern, int *occ) {
     return e;
 }
 
-template <int GEOM, bool LUT>
+template <int GEOM, int LUT>
 cudaError_t setup_march(bool idx64, bool per, int *occ) {
     if (per) return idx64 ? setup_kernel(march_kernel<GEOM, long long, true, LUT>, occ) : setup_kernel(march_kernel<GEOM, int, true, LUT>, occ);
     return idx64 ? setup_kernel(march_kernel<GEOM, long long, false, LUT>, occ) : setup_kernel(march_kernel<GEOM, int, false, LUT>, occ);
@@ -242,14 +244,16 @@ cudaError_t setup_march(bool idx64, bool per, int *occ) {
 
 // Q(tau_0) of a black body above the H I threshold (PAPER.md:85-95 with sigma ~ nu^-3, R37/R39), by composite
 // Simpson in v = nu_0 / nu on (0, 1]:  int_{x0}^inf B(x) (1 - exp(-tau (x0/x)^3)) dx,  B = x^2 / (e^x - 1), x = x0 / v.
-double bb_absorbed(double x0, double tau, bool with_abs) {
+// mode 0: the norm int B dx; 1: Q; 2: T = dQ/dtau_0 = int B (x0/x)^3 exp(-tau (x0/x)^3) dx (R40)
+double bb_absorbed(double x0, double tau, int mode) {
     const int N = 40000;
     double sum = 0.0;
     for (int i = 1; i <= N; ++i) {                                          // v = 0: the integrand vanishes
         const double v = (double)i / (double)N;
         const double x = x0 / v;
         double f = x * x * std::exp(-x) / -std::expm1(-x) * (x0 / (v * v));
-        if (with_abs) f *= -std::expm1(-tau * v * v * v);
+        if (mode == 1) f *= -std::expm1(-tau * v * v * v);
+        if (mode == 2) f *= (v * v * v) * std::exp(-tau * v * v * v);
         sum += (i == N ? 1.0 : ((i & 1) ? 4.0 : 2.0)) * f;
     }
     return sum / (3.0 * (double)N);
@@ -396,14 +400,16 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     int occ = 0;
     if (e == cudaSuccess) {
         switch (geom_template(p.geom_mode)) {
-            case 0: e = setup_march<0, false>(ctx->idx64, g.periodic != 0, &occ); break;
-            case 1: e = setup_march<1, false>(ctx->idx64, g.periodic != 0, &occ); break;
-            case 4: e = setup_march<4, false>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 0: e = setup_march<0, 0>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 1: e = setup_march<1, 0>(ctx->idx64, g.periodic != 0, &occ); break;
+            case 4: e = setup_march<4, 0>(ctx->idx64, g.periodic != 0, &occ); break;
             default: {
-                int occ_lut = 0;
-                e = setup_march<3, true>(ctx->idx64, g.periodic != 0, &occ_lut);
-                if (e == cudaSuccess) e = setup_march<3, false>(ctx->idx64, g.periodic != 0, &occ);
+                int occ_lut = 0, occ_thin = 0;
+                e = setup_march<3, 1>(ctx->idx64, g.periodic != 0, &occ_lut);
+                if (e == cudaSuccess) e = setup_march<3, 2>(ctx->idx64, g.periodic != 0, &occ_thin);
+                if (e == cudaSuccess) e = setup_march<3, 0>(ctx->idx64, g.periodic != 0, &occ);
                 if (occ_lut < occ) occ = occ_lut;
+                if (occ_thin < occ) occ = occ_thin;
                 break;
             }
         }
@@ -428,6 +434,7 @@ void nyxrt_destroy(nyxrt_ctx *ctx) {
     for (int k = 0; k < 4; ++k)
         if (ctx->tev[k]) cudaEventDestroy(ctx->tev[k]);
     if (ctx->d_lut) cudaFree(ctx->d_lut);
+    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->h_ls) cudaFreeHost(ctx->h_ls);
     if (ctx->h_ds) cudaFreeHost(ctx->h_ds);
@@ -583,6 +590,10 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         a.lut_fscale = std::ldexp(1.0, -a.lut_fb);
         a.lut_fmask = (1ll << a.lut_fb) - 1;
         a.lut_k0 = (long long)(ctx->lut_e_lo + 1023) << ctx->lut_m;
+        a.lut_t = ctx->d_lut_t;
+        a.lut_t_first = ctx->lut_t_first;
+        a.lut_t_last = ctx->lut_t_last;
+        a.tau_thin = ctx->tau_thin;
     }
     const int gt = geom_template(ctx->p.geom_mode);
     const int emit_blocks = ctx->sm_count * 4;
@@ -602,12 +613,13 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
             switch (gt) {
-                case 0: launch_march<0, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
-                case 1: launch_march<1, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
-                case 4: launch_march<4, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 0: launch_march<0, 0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 1: launch_march<1, 0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
+                case 4: launch_march<4, 0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
                 default:
-                    if (lut) launch_march<3, true>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
-                    else launch_march<3, false>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
+                    if (lut && ctx->d_lut_t) launch_march<3, 2>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
+                    else if (lut) launch_march<3, 1>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
+                    else launch_march<3, 0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st);
                     break;
             }
             CU(cudaEventRecord(ctx->mev[2 * n_launch + 1], st));
@@ -691,6 +703,8 @@ int nyxrt_spectrum_node_tau(int32_t e_lo, int32_t m, int64_t k, double *tau) {
 int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, const double *h_q, int64_t n) {
     if (!ctx) return NYXRT_EINVAL;
     CU(cudaSetDevice(ctx->g.device));
+    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);                              // a new Q table drops the thin table
+    ctx->d_lut_t = nullptr;
     if (!h_q) {                                                            // back to monochromatic
         if (ctx->d_lut) cudaFree(ctx->d_lut);
         ctx->d_lut = nullptr;
@@ -720,15 +734,52 @@ int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, co
     return NYXRT_OK;
 }
 
+int nyxrt_set_spectrum_thin(nyxrt_ctx *ctx, const double *h_t, int64_t n, double tau_thin) {
+    if (!ctx) return NYXRT_EINVAL;
+    CU(cudaSetDevice(ctx->g.device));
+    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
+    ctx->d_lut_t = nullptr;
+    if (!h_t) return NYXRT_OK;
+    if (!ctx->d_lut) return fail(ctx, NYXRT_ESTATE, "set_spectrum_thin: set the Q table first");
+    if (n != ctx->lut_n || !(tau_thin >= 0.0)) return fail(ctx, NYXRT_EINVAL, "set_spectrum_thin: bad length or threshold");
+    for (int64_t k = 0; k < n; ++k)
+        if (!(h_t[k] >= 0.0) || !(h_t[k] <= 1.0e300)) return fail(ctx, NYXRT_EINVAL, "set_spectrum_thin: T must be finite and >= 0");
+    double *d = nullptr;
+    CU(cudaMalloc(&d, n * sizeof(double)));
+    const cudaError_t ce = cudaMemcpy(d, h_t, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (ce != cudaSuccess) {
+        cudaFree(d);
+        return fail(ctx, NYXRT_ECUDA, "set_spectrum_thin: copy failed: %s", cudaGetErrorString(ce));
+    }
+    ctx->d_lut_t = d;
+    ctx->lut_t_first = h_t[0];
+    ctx->lut_t_last = h_t[n - 1];
+    ctx->tau_thin = tau_thin;
+    return NYXRT_OK;
+}
+
+int nyxrt_blackbody_thin_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_t, int64_t n) {
+    int64_t need = 0;
+    if (!h_t || !(t_eff_K > 0.0) || nyxrt_spectrum_nodes(e_lo, e_hi, m, &need) != NYXRT_OK || n != need) return NYXRT_EINVAL;
+    const double x0 = 13.598434 * 1.602176634e-19 / (1.380649e-23 * t_eff_K);   // h nu_0 / k T_eff
+    const double norm = bb_absorbed(x0, 0.0, 0);
+    for (int64_t k = 0; k < n; ++k) {
+        double tau = 0.0;
+        nyxrt_spectrum_node_tau(e_lo, m, k, &tau);
+        h_t[k] = bb_absorbed(x0, tau, 2) / norm;
+    }
+    return NYXRT_OK;
+}
+
 int nyxrt_blackbody_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_q, int64_t n) {
     int64_t need = 0;
     if (!h_q || !(t_eff_K > 0.0) || nyxrt_spectrum_nodes(e_lo, e_hi, m, &need) != NYXRT_OK || n != need) return NYXRT_EINVAL;
     const double x0 = 13.598434 * 1.602176634e-19 / (1.380649e-23 * t_eff_K);   // h nu_0 / k T_eff
-    const double norm = bb_absorbed(x0, 0.0, false);
+    const double norm = bb_absorbed(x0, 0.0, 0);
     for (int64_t k = 0; k < n; ++k) {
         double tau = 0.0;
         nyxrt_spectrum_node_tau(e_lo, m, k, &tau);
-        const double q = bb_absorbed(x0, tau, true) / norm;
+        const double q = bb_absorbed(x0, tau, 1) / norm;
         h_q[k] = q > 1.0 ? 1.0 : q;
         if (k > 0 && h_q[k] < h_q[k - 1]) h_q[k] = h_q[k - 1];              // quadrature noise near Q = 1
     }

@@ -67,6 +67,8 @@ struct MarchArgs {
                                          // cells = sqrt(3) L_box for a cube
     // spectrum table, used by the LUT instantiations only
     const double *lut_q;                 // Q at the nodes
+    const double *lut_t;                 // T = dQ/dtau_0 at the nodes (thin segments), or null
+    double lut_t_first, lut_t_last, tau_thin;
     double lut_t_lo, lut_t_hi, lut_inv_t_lo, lut_q_first, lut_q_last, lut_fscale;
     long long lut_k0, lut_fmask;
     int lut_fb;

@@ -75,7 +75,7 @@ EXPORTS = ["nyxrt_create", "nyxrt_workspace_bytes", "nyxrt_set_workspace", "nyxr
            "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats",
            "nyxrt_timestep", "nyxrt_sizeof_ode", "nyxrt_sizeof_tstats", "nyxrt_set_shard", "nyxrt_trace_photons",
            "nyxrt_finalise", "nyxrt_spectrum_nodes", "nyxrt_spectrum_node_tau", "nyxrt_set_spectrum",
-           "nyxrt_blackbody_table"]
+           "nyxrt_blackbody_table", "nyxrt_set_spectrum_thin", "nyxrt_blackbody_thin_table"]
 
 _lib = None
 
@@ -197,6 +197,25 @@ def nyxrt_blackbody_table(t_eff_K, e_lo, e_hi, m):
     if rc != OK:
         raise NyxrtError(rc, "blackbody_table: bad argument")
     return q
+
+
+def nyxrt_set_spectrum_thin(ctx, t=None, tau_thin=0.0):
+    """t: host array of T = dQ/dtau_0 at the nodes of the Q table (None: thin table off)."""
+    if t is None:
+        _check(ctx, lib().nyxrt_set_spectrum_thin(ctx, None, C.c_int64(0), C.c_double(0.0)))
+        return
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    _check(ctx, lib().nyxrt_set_spectrum_thin(ctx, t.ctypes.data_as(C.c_void_p), C.c_int64(len(t)), C.c_double(tau_thin)))
+
+
+def nyxrt_blackbody_thin_table(t_eff_K, e_lo, e_hi, m):
+    n = nyxrt_spectrum_nodes(e_lo, e_hi, m)
+    t = np.zeros(n)
+    rc = lib().nyxrt_blackbody_thin_table(C.c_double(t_eff_K), C.c_int32(e_lo), C.c_int32(e_hi), C.c_int32(m),
+                                          t.ctypes.data_as(C.c_void_p), C.c_int64(n))
+    if rc != OK:
+        raise NyxrtError(rc, "blackbody_thin_table: bad argument")
+    return t
 
 
 def nyxrt_set_shard(ctx, rank, world):
@@ -351,6 +370,9 @@ class Tracer:
 
     def set_spectrum(self, e_lo=0, e_hi=0, m=0, q=None):
         nyxrt_set_spectrum(self.ctx, e_lo, e_hi, m, q)
+
+    def set_spectrum_thin(self, t=None, tau_thin=0.0):
+        nyxrt_set_spectrum_thin(self.ctx, t, tau_thin)
 
     def set_shard(self, rank, world):
         nyxrt_set_shard(self.ctx, rank, world)
