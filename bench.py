@@ -52,6 +52,9 @@ def parse():
     ap.add_argument("--timestep-myr", type=float, default=0.0,
                     help="time a whole RT timestep of this length (iterative RT<->ODE solve, nyxrt_timestep) instead of one RT step")
     ap.add_argument("--periodic", action="store_true", help="periodic box (default: BASELINE.json's open box)")
+    ap.add_argument("--graph-loop", action="store_true",
+                    help="time the production loop (one CUDA-graph launch per trace; no per-launch events, so the "
+                         "roofline's achieved figure then uses the loop time instead of the march launches' own)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -250,7 +253,9 @@ def main():
     cfg, pos, L = make_workload(args, "cuda")
     nH, xHI = cfg["nH"], cfg["xHI"]
     fdt = "f32" if nH.dtype == torch.float32 else "f64"
-    tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], cfg["params"], field_dtype=nH.dtype, max_sources=len(L),
+    params = dict(cfg["params"])
+    params["flags"] = 0 if args.graph_loop else nyxrt.FLAG_LAUNCH_TIMING    # per-launch events: what the roofline needs
+    tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], params, field_dtype=nH.dtype, max_sources=len(L),
                       batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local,
                       periodic=1 if args.periodic else 0)
     if args.spectrum_teff > 0:
@@ -312,7 +317,7 @@ def main():
         st = step()
         seg += st.segments
         nbr += st.neighbour_deposits
-        ms_march += st.ms_march
+        ms_march += st.ms_march if not args.graph_loop else st.ms_loop
         launches += st.kernel_launches + 3            # + prep_fields, sum_partials, snap
         march_launches += st.march_launches
     e1.record(stream)
@@ -413,6 +418,8 @@ def main():
                                periodic=bool(args.periodic), timestep=getattr(st, "timestep", None),
                                spectrum=("black body %g K, tau_0 table 2^-20..2^12, 256 nodes per octave" % args.spectrum_teff)
                                if args.spectrum_teff > 0 else "monochromatic"),
+                   loop="one CUDA-graph launch per trace (WHILE node over sched -> emit -> march)" if args.graph_loop
+                   else "host-enqueued launches with a CUDA-event pair around every march launch (NYXRT_FLAG_LAUNCH_TIMING)",
                    rt_step_ms=ms / args.steps, march_ms_per_step=ms_march / args.steps,
                    gpu_launches=int(launches), clocks=clk, e2e=e2e, roofline=roof, cpu_baseline=cpu,
                    stats=dict(iterations=int(st.iterations), peak_pool_rays=int(st.peak_pool_rays),

@@ -36,6 +36,12 @@ extern "C" {
 
 #define NYXRT_MAXLEV 16
 
+/* nyxrt_params.flags */
+#define NYXRT_FLAG_LAUNCH_TIMING 1   /* profiling mode: the ray loop is enqueued launch by launch from the host with a
+                                        pair of CUDA events around every march launch (stats ms_march); without it the
+                                        loop runs as one CUDA-graph launch (a WHILE node over sched -> emit -> march) and
+                                        ms_march is 0.  Same kernels, same results. */
+
 typedef struct nyxrt_ctx nyxrt_ctx;      /* opaque */
 
 /* The coarse RT grid ("downsampled onto a coarse grid"; cubic cells). */
@@ -72,7 +78,7 @@ typedef struct {
     int32_t merge;             /* 0 off, 1 on, 2 automerge                           */
     int32_t n_min_samples;     /* N_min of PAPER.md:317                                             */
     int32_t samp_level;        /* HEALPix level of the shell sample pattern, 12*4^level dirs (R6)   */
-    int32_t reserved;          /* 0                                                                 */
+    int32_t flags;             /* NYXRT_FLAG_* (0: production)                                      */
 } nyxrt_params;
 
 /* Filled by nyxrt_trace (host memory).  Per-level arrays are indexed by HEALPix level l. */

@@ -36,8 +36,7 @@ constexpr int MARCH_CARVEOUT = 40;       // preferred shared-memory carve-out [%
 //   2. if sources remain, top level 0 up with 12 rays per source, then 1. again; else
 //   3. the shallowest non-empty level (drain).
 // With caps of 2B (level 0) and 5B + slab slack (deeper levels) no stack can overflow.
-__global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__device__ __forceinline__ void sched_decide(LoopState *ls, DevStats *ds, const RayPool &pool, int nlev) {
     ls->emit_n = 0;
     ls->batch = 0;
     ls->fetch = 0;
@@ -81,6 +80,15 @@ __global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev
     ls->seg_round = pick < 2 ? 3 : 21;
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
+}
+
+// `cond`: the handle of the CUDA-graph WHILE node that wraps sched -> emit -> march when the loop runs as one graph
+// launch (nyxrt.cu); the loop goes on while it is non-zero.  use_cond = 0: launched from the host loop.
+__global__ void sched_kernel(LoopState *ls, DevStats *ds, RayPool pool, int nlev, cudaGraphConditionalHandle cond,
+                             int use_cond) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    sched_decide(ls, ds, pool, nlev);
+    if (use_cond) cudaGraphSetConditional(cond, ls->done ? 0u : 1u);
 }
 
 // ---------------------------------------------------------------------------------------------------

@@ -83,6 +83,12 @@ struct nyxrt_ctx {
     cudaEvent_t *mev;                      // pairs of events around every march launch
     long long mev_cap;
     cudaStream_t own_stream;
+    // the ray loop as one CUDA-graph launch: WHILE node over sched -> emit -> march (rebuilt when its arguments change)
+    cudaGraph_t loop_graph;
+    cudaGraphExec_t loop_exec;
+    MarchArgs loop_args;
+    int loop_rank, loop_world;
+    const void *loop_fn;
     LoopState *h_ls;                       // pinned
     DevStats *h_ds;                        // pinned
     double *h_scalars;                     // pinned
@@ -261,6 +267,77 @@ double bb_absorbed(double x0, double tau, int mode) {
 
 int geom_template(int mode) { return mode == 2 ? 3 : mode; }
 
+template <int GEOM, int LUT>
+const void *march_fn_of(bool idx64, bool per) {
+    if (per) return idx64 ? (const void *)march_kernel<GEOM, long long, true, LUT> : (const void *)march_kernel<GEOM, int, true, LUT>;
+    return idx64 ? (const void *)march_kernel<GEOM, long long, false, LUT> : (const void *)march_kernel<GEOM, int, false, LUT>;
+}
+
+const void *march_fn(int gt, bool idx64, bool per, int lut) {
+    switch (gt) {
+        case 0: return march_fn_of<0, 0>(idx64, per);
+        case 1: return march_fn_of<1, 0>(idx64, per);
+        case 4: return march_fn_of<4, 0>(idx64, per);
+        default: return lut == 2 ? march_fn_of<3, 2>(idx64, per) : (lut == 1 ? march_fn_of<3, 1>(idx64, per) : march_fn_of<3, 0>(idx64, per));
+    }
+}
+
+void drop_loop_graph(nyxrt_ctx *c) {
+    if (c->loop_exec) cudaGraphExecDestroy(c->loop_exec);
+    if (c->loop_graph) cudaGraphDestroy(c->loop_graph);
+    c->loop_exec = nullptr;
+    c->loop_graph = nullptr;
+}
+
+// The ray loop of DESIGN.md rows a4-a8 as ONE graph: a conditional WHILE node whose body is sched -> emit -> march;
+// sched_kernel keeps the condition at "rays or sources are left" (cudaGraphSetConditional), so the device iterates
+// without the host and stops after the first empty round.  Kernel arguments are baked into the nodes: the graph is
+// rebuilt when they change (new spectrum table, shard, workspace).
+cudaError_t build_loop_graph(nyxrt_ctx *c, const MarchArgs &a, const void *fn, const double *cat_L, int emit_blocks) {
+    drop_loop_graph(c);
+    cudaError_t e = cudaGraphCreate(&c->loop_graph, 0);
+    if (e != cudaSuccess) return e;
+    cudaGraphConditionalHandle cond;
+    e = cudaGraphConditionalHandleCreate(&cond, c->loop_graph, 1, cudaGraphCondAssignDefault);
+    if (e != cudaSuccess) return e;
+    cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
+    cp.type = cudaGraphNodeTypeConditional;
+    cp.conditional.handle = cond;
+    cp.conditional.type = cudaGraphCondTypeWhile;
+    cp.conditional.size = 1;
+    cudaGraphNode_t wnode;
+    e = cudaGraphAddNode(&wnode, c->loop_graph, nullptr, 0, &cp);
+    if (e != cudaSuccess) return e;
+    cudaGraph_t body = cp.conditional.phGraph_out[0];
+    cudaGraphNode_t n_sched, n_emit, n_march;
+    int use_cond = 1, nlev = c->nlev, rank = c->shard_rank, world = c->shard_world;
+    LoopState *ls = c->ls;
+    DevStats *ds = c->ds;
+    RayPool pool = c->pool;
+    MarchArgs args = a;
+    void *p_sched[] = {&ls, &ds, &pool, &nlev, &cond, &use_cond};
+    void *p_emit[] = {&ls, &pool, &cat_L, &rank, &world};
+    void *p_march[] = {&args};
+    cudaKernelNodeParams kp;
+    memset(&kp, 0, sizeof kp);
+    kp.func = (void *)sched_kernel; kp.gridDim = dim3(1); kp.blockDim = dim3(32); kp.kernelParams = p_sched;
+    e = cudaGraphAddKernelNode(&n_sched, body, nullptr, 0, &kp);
+    if (e != cudaSuccess) return e;
+    kp.func = (void *)emit_kernel; kp.gridDim = dim3(emit_blocks); kp.blockDim = dim3(256); kp.kernelParams = p_emit;
+    e = cudaGraphAddKernelNode(&n_emit, body, &n_sched, 1, &kp);
+    if (e != cudaSuccess) return e;
+    kp.func = const_cast<void *>(fn); kp.gridDim = dim3(c->march_blocks); kp.blockDim = dim3(MARCH_THREADS); kp.kernelParams = p_march;
+    e = cudaGraphAddKernelNode(&n_march, body, &n_emit, 1, &kp);
+    if (e != cudaSuccess) return e;
+    e = cudaGraphInstantiate(&c->loop_exec, c->loop_graph, 0);
+    if (e != cudaSuccess) return e;
+    c->loop_args = a;
+    c->loop_rank = rank;
+    c->loop_world = world;
+    c->loop_fn = fn;
+    return cudaSuccess;
+}
+
 // ---- source pass: dedup + sort, optional radius + merge -------------------------------------------
 int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     SrcBufs &s = ctx->sb;
@@ -274,16 +351,22 @@ int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     while (((long long)1 << key_bits) < ctx->ncell) ++key_bits;
     size_t tb = s.cub_bytes;
     // (a1) stable sort by cell key, run heads, sequential flux sums
-    iota_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.idx_a, n);
-    CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.key_a, s.key_b, s.idx_a, s.idx_b, (int)n, 0, key_bits, st));
-    head_flags_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.key_b, n, s.flag);
-    tb = s.cub_bytes;
-    CU(cub::DeviceScan::InclusiveSum(s.cub_tmp, tb, s.flag, s.gid, (int)n, st));
+    if (n == 1) {
+        single_source_kernel<<<1, 32, 0, st>>>(s.key_a, s.key_b, s.idx_b, s.flag, s.gid);   // the sorted order of one source
+    } else {
+        iota_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.idx_a, n);
+        CU(cub::DeviceRadixSort::SortPairs(s.cub_tmp, tb, s.key_a, s.key_b, s.idx_a, s.idx_b, (int)n, 0, key_bits, st));
+        head_flags_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.key_b, n, s.flag);
+        tb = s.cub_bytes;
+        CU(cub::DeviceScan::InclusiveSum(s.cub_tmp, tb, s.flag, s.gid, (int)n, st));
+    }
     dedup_kernel<<<blocks_for(n, 256), 256, 0, st>>>(s.key_b, s.idx_b, s.flag, s.gid, n, s.L, gd, s.cell[0], s.L2[0],
                                                       s.ckey[0]);
-    int nd = 0;
-    CU(cudaMemcpyAsync(&nd, s.gid + (n - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    int nd = 1;                                                    // one source: one catalogue entry, no need to ask
+    if (n > 1) {
+        CU(cudaMemcpyAsync(&nd, s.gid + (n - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
     ctx->n_dedup = ctx->n_cat = nd;
     fill_double_kernel<<<blocks_for(nd, 256), 256, 0, st>>>(s.r[0], nd, 0.0);
     if (!do_merge) return NYXRT_OK;
@@ -331,9 +414,11 @@ int source_pass(nyxrt_ctx *ctx, cudaStream_t st, bool do_merge) {
     collapse_big_kernel<<<ctx->sm_count * 2, 32 * COLLAPSE_WARPS, 0, st>>>(s.lab_b, s.gid, nd, s.m_cell, s.m_L, s.m_r, gd,
                                                                           s.cell[1], s.L2[1], s.r[1], s.ckey[1], s.bin_a,
                                                                           s.bad + 1);
-    int nm = 0;
-    CU(cudaMemcpyAsync(&nm, s.gid + (nd - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
+    int nm = 1;
+    if (nd > 1) {
+        CU(cudaMemcpyAsync(&nm, s.gid + (nd - 1), sizeof(int), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
     // final sort by cell key; keys are unique
     iota_kernel<<<blocks_for(nm, 256), 256, 0, st>>>(s.idx_a, nm);
     tb = s.cub_bytes;
@@ -427,6 +512,7 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
 
 void nyxrt_destroy(nyxrt_ctx *ctx) {
     if (!ctx) return;
+    drop_loop_graph(ctx);
     for (long long k = 0; k < ctx->mev_cap; ++k) cudaEventDestroy(ctx->mev[k]);
     free(ctx->mev);
     for (int k = 0; k < 4; ++k)
@@ -597,11 +683,20 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     }
     const int gt = geom_template(ctx->p.geom_mode);
     const int emit_blocks = ctx->sm_count * 4;
+    const bool timing = (ctx->p.flags & NYXRT_FLAG_LAUNCH_TIMING) != 0;
     int chunk = 8;
     long long n_launch = 0;
-    for (;;) {
+    if (!timing) {
+        // production: the whole loop is one graph launch; the host synchronises once, after finalise
+        const void *fn = march_fn(gt, ctx->idx64, ctx->g.periodic != 0, lut ? (ctx->d_lut_t ? 2 : 1) : 0);
+        if (!ctx->loop_exec || fn != ctx->loop_fn || ctx->loop_rank != ctx->shard_rank || ctx->loop_world != ctx->shard_world ||
+            memcmp(&a, &ctx->loop_args, sizeof a) != 0)
+            CU(build_loop_graph(ctx, a, fn, s.L2[0], emit_blocks));
+        CU(cudaGraphLaunch(ctx->loop_exec, st));
+    }
+    for (; timing;) {
         for (int i = 0; i < chunk; ++i) {
-            sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev);
+            sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev, (cudaGraphConditionalHandle)0, 0);
             emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0], ctx->shard_rank, ctx->shard_world);
             if (n_launch + 1 > ctx->mev_cap / 2) {                       // grow the event pool
                 const long long cap = ctx->mev_cap ? 2 * ctx->mev_cap : 1024;
@@ -640,8 +735,13 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     CU(cudaEventRecord(ctx->ev[3], st));
     CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));
     CU(cudaMemcpyAsync(ctx->h_scalars, ctx->scalars, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (!timing) CU(cudaMemcpyAsync(ctx->h_ls, ctx->ls, sizeof(LoopState), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
+    if (!timing) {
+        if (ctx->h_ls->overflow) return fail(ctx, NYXRT_EOVERFLOW, "trace: ray pool overflow at level %d", ctx->h_ls->level + 1);
+        n_launch = (long long)ctx->h_ls->iterations + 1;                 // rounds of the WHILE body (the last one is empty)
+    }
     if (hs) {
         memset(hs, 0, sizeof *hs);
         const DevStats &d = *ctx->h_ds;
@@ -668,7 +768,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         cudaEventElapsedTime(&hs->ms_total, ctx->ev[0], ctx->ev[3]);
         double ms = 0.0;
         const long long live = (long long)ctx->h_ls->iterations;       // launches that had a batch
-        for (long long k = 0; k < n_launch && k < live; ++k) {
+        for (long long k = 0; timing && k < n_launch && k < live; ++k) {
             float t = 0.f;
             cudaEventElapsedTime(&t, ctx->mev[2 * k], ctx->mev[2 * k + 1]);
             ms += t;

@@ -136,6 +136,11 @@ __device__ __forceinline__ void uf_unite(int *par, int a, int b) {
     }
 }
 
+// n = 1: what the sort, the run heads and their scan would produce
+__global__ void single_source_kernel(const long long *key_a, long long *key_b, int *idx_b, int *flag, int *gid) {
+    if (threadIdx.x == 0) { key_b[0] = key_a[0]; idx_b[0] = 0; flag[0] = 1; gid[0] = 1; }
+}
+
 __global__ void iota_kernel(int *p, long long n) {
     const long long a = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (a < n) p[a] = (int)a;

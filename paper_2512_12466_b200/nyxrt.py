@@ -12,6 +12,7 @@ from . import build as _build
 
 MAXLEV = 16
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EOVERFLOW = 0, -1, -2, -3, -4, -5
+FLAG_LAUNCH_TIMING = 1
 _ERRNAME = {EINVAL: "NYXRT_EINVAL", ESTATE: "NYXRT_ESTATE", ENOMEM: "NYXRT_ENOMEM", ECUDA: "NYXRT_ECUDA",
             EOVERFLOW: "NYXRT_EOVERFLOW"}
 
@@ -34,7 +35,7 @@ class nyxrt_params(C.Structure):
                 ("delta_r", C.c_double), ("r_max", C.c_double), ("f_ov", C.c_double), ("x_th", C.c_double),
                 ("f_req", C.c_double), ("eps", C.c_double),
                 ("level_max", C.c_int32), ("geom_mode", C.c_int32), ("merge", C.c_int32),
-                ("n_min_samples", C.c_int32), ("samp_level", C.c_int32), ("reserved", C.c_int32)]
+                ("n_min_samples", C.c_int32), ("samp_level", C.c_int32), ("flags", C.c_int32)]
 
 
 class nyxrt_stats(C.Structure):

@@ -214,3 +214,36 @@ def test_merge_large_groups(O, periodic):
     rgb = run_gpu(cfgb, batch_rays=16384, periodic=periodic)
     compare(rgb, run_oracle(O, cfgb, periodic=periodic), cfgb)
     assert 10 < rgb[2].n_src_merged < rgb[2].n_src_dedup
+
+
+def test_graph_loop_and_profiling_loop_are_the_same_step(O):
+    """Production runs the ray loop as one CUDA-graph launch (WHILE node over sched -> emit -> march); with
+    NYXRT_FLAG_LAUNCH_TIMING the host enqueues the same kernels launch by launch with an event pair around every
+    march launch (what bench.py's roofline needs).  Same counters, same rates, and both match the oracle; several
+    traces on one context reuse the graph, a new spectrum table or shard rebuilds it."""
+    from paper_2512_12466_b200 import nyxrt
+    cfg = synth.make(4, n=64, n_src=3000)
+    worst, rg, ro = both(O, cfg, batch_rays=16384)
+    worst_t, rt, _ = both(O, cfg, params=dict(flags=nyxrt.FLAG_LAUNCH_TIMING), batch_rays=16384)
+    sg, st = rg[2], rt[2]
+    for name in ("spawned", "split", "killed_tau", "exited"):
+        assert list(getattr(sg, name)) == list(getattr(st, name))
+    assert sg.segments == st.segments and sg.iterations == st.iterations and sg.iterations > 10
+    assert sg.ms_march == 0.0 and st.ms_march > 0.0 and sg.march_launches == st.march_launches
+    assert np.all(np.abs(rg[0] - rt[0]) <= 1e-12 * rt[0])
+    # one context, several traces: the graph is reused, then rebuilt for a shard, and reused again
+    tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], cfg["params"], field_dtype=cfg["nH"].dtype, max_sources=len(cfg["src_L"]),
+                      batch_rays=16384)
+    try:
+        tr.set_fields(cfg["nH"].cuda(), cfg["xHI"].cuda())
+        tr.set_sources(cfg["src_pos"].numpy(), cfg["src_L"].numpy())
+        seg = [tr.trace()[2].segments for _ in range(3)]
+        tr.set_shard(0, 2)
+        s0 = tr.trace_photons()[1].segments
+        tr.set_shard(1, 2)
+        s1 = tr.trace_photons()[1].segments
+        tr.set_shard(0, 1)
+        seg.append(tr.trace()[2].segments)
+    finally:
+        tr.close()
+    assert seg == [sg.segments] * 4 and s0 + s1 == sg.segments and 0 < s0 < sg.segments
