@@ -28,6 +28,9 @@ constexpr int MARCH_THREADS = 128;
 constexpr int MARCH_WARPS = MARCH_THREADS / 32;
 constexpr int MARCH_MIN_BLOCKS = 4;      // 16 warps per SM at <= 128 registers, no spills (checked with -Xptxas -v); a fifth
                                          // block (96 registers, 132 KB of shared memory) measured 6 % slower
+#ifndef MARCH_SEG_ROUND
+#define MARCH_SEG_ROUND 21                // cells a lane marches between two retire / refill passes (15 and 30: within 0.7 %)
+#endif
 constexpr int MARCH_CARVEOUT = 40;       // preferred shared-memory carve-out [% of 228 KB]: 4 blocks x 21 KB
 
 // ---------------------------------------------------------------------------------------------------
@@ -77,7 +80,7 @@ __device__ __forceinline__ void sched_decide(LoopState *ls, DevStats *ds, const 
     ls->level = pick;
     ls->begin = pool.off[pick] + ls->count[pick];
     ls->batch = b;
-    ls->seg_round = pick < 2 ? 3 : 21;
+    ls->seg_round = pick < 2 ? 3 : MARCH_SEG_ROUND;
     ls->iterations += 1;
     ds->spawned[pick] += (unsigned long long)b;          // every slot is popped exactly once (holes subtracted later)
 }
