@@ -49,6 +49,8 @@ def parse():
                     help="N > 1: every rank runs the whole step on its own GPU (no sharding, redundant work)")
     ap.add_argument("--spectrum-teff", type=float, default=0.0,
                     help="trace with the tau_0 lookup table of a black body of this temperature [K] (default: monochromatic)")
+    ap.add_argument("--tau-thin", type=float, default=0.0,
+                    help="with --spectrum-teff: also set the table for thin segments (PAPER.md:267 footnote 3), used below this dtau_0")
     ap.add_argument("--timestep-myr", type=float, default=0.0,
                     help="time a whole RT timestep of this length (iterative RT<->ODE solve, nyxrt_timestep) instead of one RT step")
     ap.add_argument("--periodic", action="store_true", help="periodic box (default: BASELINE.json's open box)")
@@ -177,7 +179,7 @@ def oracle_sample(cfg, pos, L, budget_s, n_proc=0):
     p = O.make_params(**cfg["params"])
     model, cores = cpu_info()
     grid_bytes = nH.size * 8
-    n_proc = n_proc or max(1, min(cores, int(0.8 * psutil.virtual_memory().available // (grid_bytes + 2 ** 28))))
+    n_proc = n_proc or max(1, min(cores, len(L), int(0.8 * psutil.virtual_memory().available // (grid_bytes + 2 ** 28))))
     n, best = min(len(L), 4 * n_proc), None
     while True:
         t0 = time.perf_counter()
@@ -260,6 +262,8 @@ def main():
                       periodic=1 if args.periodic else 0)
     if args.spectrum_teff > 0:
         tr.set_spectrum(-20, 12, 8, nyxrt.nyxrt_blackbody_table(args.spectrum_teff, -20, 12, 8))
+        if args.tau_thin > 0:
+            tr.set_spectrum_thin(nyxrt.nyxrt_blackbody_thin_table(args.spectrum_teff, -20, 12, 8), args.tau_thin)
     gam = torch.empty(cfg["shape"], dtype=torch.float64, device="cuda")
     heat = torch.empty_like(gam)
     stream = torch.cuda.current_stream()
@@ -416,7 +420,8 @@ def main():
                                   % ((2 * nH.numel() * nH.element_size() + 16 * nH.numel()) / 1e9),
                                multi_gpu="sharded by source, one all-reduce of the photon grid" if args.shard else "replicas only",
                                periodic=bool(args.periodic), timestep=getattr(st, "timestep", None),
-                               spectrum=("black body %g K, tau_0 table 2^-20..2^12, 256 nodes per octave" % args.spectrum_teff)
+                               spectrum=("black body %g K, tau_0 table 2^-20..2^12, 256 nodes per octave%s" % (
+                                   args.spectrum_teff, ", thin table below dtau_0 = %g" % args.tau_thin if args.tau_thin > 0 else ""))
                                if args.spectrum_teff > 0 else "monochromatic"),
                    loop="one CUDA-graph launch per trace (WHILE node over sched -> emit -> march)" if args.graph_loop
                    else "host-enqueued launches with a CUDA-event pair around every march launch (NYXRT_FLAG_LAUNCH_TIMING)",

@@ -61,7 +61,10 @@ class _Stats:
 
 @pytest.mark.parametrize("periodic", [0, 1])
 def test_two_processes_one_allreduce(O, periodic):
+    import gc
     world = 2
+    gc.collect()
+    torch.cuda.empty_cache()          # the children need room for their own contexts next to this process's cache
     with tempfile.TemporaryDirectory() as tmp:
         mp.spawn(_worker, args=(world, 29541 + periodic, tmp, periodic), nprocs=world, join=True)
         r = [np.load(os.path.join(tmp, "rank%d.npz" % k)) for k in range(world)]
