@@ -89,7 +89,10 @@ struct nyxrt_ctx {
     MarchArgs loop_args;
     int loop_rank, loop_world;
     const void *loop_fn;
+    cudaGraphNode_t loop_finalise;         // the finalise node: its output pointers are patched when they change
+    double *loop_gamma, *loop_heat, *loop_photons;
     LoopState *h_ls;                       // pinned
+    LoopState *h_ls_init;                  // pinned: the loop state a trace starts from (read by the graph's copy node)
     DevStats *h_ds;                        // pinned
     double *h_scalars;                     // pinned
 };
@@ -289,25 +292,56 @@ void drop_loop_graph(nyxrt_ctx *c) {
     c->loop_graph = nullptr;
 }
 
-// The ray loop of DESIGN.md rows a4-a8 as ONE graph: a conditional WHILE node whose body is sched -> emit -> march;
-// sched_kernel keeps the condition at "rays or sources are left" (cudaGraphSetConditional), so the device iterates
-// without the host and stops after the first empty round.  Kernel arguments are baked into the nodes: the graph is
-// rebuilt when they change (new spectrum table, shard, workspace).
-cudaError_t build_loop_graph(nyxrt_ctx *c, const MarchArgs &a, const void *fn, const double *cat_L, int emit_blocks) {
+// Everything of a trace after the source pass as ONE graph launch (DESIGN.md rows a4-a9): clear the accumulator and
+// the counters, copy the initial loop state, a conditional WHILE node whose body is sched -> emit -> march
+// (sched_kernel keeps the condition at "rays or sources are left", cudaGraphSetConditional: the device iterates
+// without the host and stops after the first empty round), finalise, and the copies of the counters back to pinned
+// host memory.  Kernel arguments are baked into the nodes: the graph is rebuilt when they change (new spectrum
+// table, shard, workspace); only the output pointers of finalise are patched in place.
+struct FinaliseParams {
+    double *gamma, *heat;
+    const double *acc, *absorber;
+    int nx, ny, nz;
+    double V, e_excess;
+    int periodic;
+    double *photons, *partial;
+};
+
+cudaError_t set_finalise_params(nyxrt_ctx *c, cudaGraph_t g, cudaGraphNode_t *node, cudaGraphNode_t dep, double *gamma,
+                                double *heat, double *photons) {
+    FinaliseParams f{gamma, heat, c->acc, c->absorber, c->g.nx, c->g.ny, c->g.nz, c->g.dx_cm * c->g.dx_cm * c->g.dx_cm,
+                     c->p.e_excess_erg, c->g.periodic, photons, c->partial};
+    void *p[] = {&f.gamma, &f.heat, &f.acc, &f.absorber, &f.nx, &f.ny, &f.nz, &f.V, &f.e_excess, &f.periodic, &f.photons, &f.partial};
+    cudaKernelNodeParams kp;
+    memset(&kp, 0, sizeof kp);
+    kp.func = (void *)finalise_kernel; kp.gridDim = dim3(NPARTIAL); kp.blockDim = dim3(256); kp.kernelParams = p;
+    c->loop_gamma = gamma; c->loop_heat = heat; c->loop_photons = photons;
+    if (g) return cudaGraphAddKernelNode(node, g, &dep, 1, &kp);
+    return cudaGraphExecKernelNodeSetParams(c->loop_exec, *node, &kp);
+}
+
+cudaError_t build_loop_graph(nyxrt_ctx *c, const MarchArgs &a, const void *fn, const double *cat_L, int emit_blocks,
+                             double *gamma, double *heat, double *photons) {
     drop_loop_graph(c);
     cudaError_t e = cudaGraphCreate(&c->loop_graph, 0);
     if (e != cudaSuccess) return e;
+    cudaGraph_t G = c->loop_graph;
+    cudaGraphNode_t n_clear, n_stats, n_state, n_while, n_ev2, n_sum, n_ev3, n_c1, n_c2, n_c3;
+    cudaMemsetParams mp;
+    memset(&mp, 0, sizeof mp);
+    mp.dst = c->acc; mp.value = 0; mp.elementSize = 4; mp.width = (size_t)c->pcell * 2; mp.height = 1; mp.pitch = mp.width * 4;
+    if ((e = cudaGraphAddMemsetNode(&n_clear, G, nullptr, 0, &mp)) != cudaSuccess) return e;
+    mp.dst = c->ds; mp.width = sizeof(DevStats) / 4; mp.pitch = sizeof(DevStats);
+    if ((e = cudaGraphAddMemsetNode(&n_stats, G, &n_clear, 1, &mp)) != cudaSuccess) return e;
+    if ((e = cudaGraphAddMemcpyNode1D(&n_state, G, &n_stats, 1, c->ls, c->h_ls_init, sizeof(LoopState), cudaMemcpyHostToDevice)) != cudaSuccess) return e;
     cudaGraphConditionalHandle cond;
-    e = cudaGraphConditionalHandleCreate(&cond, c->loop_graph, 1, cudaGraphCondAssignDefault);
-    if (e != cudaSuccess) return e;
+    if ((e = cudaGraphConditionalHandleCreate(&cond, G, 1, cudaGraphCondAssignDefault)) != cudaSuccess) return e;
     cudaGraphNodeParams cp = {cudaGraphNodeTypeConditional};
     cp.type = cudaGraphNodeTypeConditional;
     cp.conditional.handle = cond;
     cp.conditional.type = cudaGraphCondTypeWhile;
     cp.conditional.size = 1;
-    cudaGraphNode_t wnode;
-    e = cudaGraphAddNode(&wnode, c->loop_graph, nullptr, 0, &cp);
-    if (e != cudaSuccess) return e;
+    if ((e = cudaGraphAddNode(&n_while, G, &n_state, 1, &cp)) != cudaSuccess) return e;
     cudaGraph_t body = cp.conditional.phGraph_out[0];
     cudaGraphNode_t n_sched, n_emit, n_march;
     int use_cond = 1, nlev = c->nlev, rank = c->shard_rank, world = c->shard_world;
@@ -321,16 +355,23 @@ cudaError_t build_loop_graph(nyxrt_ctx *c, const MarchArgs &a, const void *fn, c
     cudaKernelNodeParams kp;
     memset(&kp, 0, sizeof kp);
     kp.func = (void *)sched_kernel; kp.gridDim = dim3(1); kp.blockDim = dim3(32); kp.kernelParams = p_sched;
-    e = cudaGraphAddKernelNode(&n_sched, body, nullptr, 0, &kp);
-    if (e != cudaSuccess) return e;
+    if ((e = cudaGraphAddKernelNode(&n_sched, body, nullptr, 0, &kp)) != cudaSuccess) return e;
     kp.func = (void *)emit_kernel; kp.gridDim = dim3(emit_blocks); kp.blockDim = dim3(256); kp.kernelParams = p_emit;
-    e = cudaGraphAddKernelNode(&n_emit, body, &n_sched, 1, &kp);
-    if (e != cudaSuccess) return e;
+    if ((e = cudaGraphAddKernelNode(&n_emit, body, &n_sched, 1, &kp)) != cudaSuccess) return e;
     kp.func = const_cast<void *>(fn); kp.gridDim = dim3(c->march_blocks); kp.blockDim = dim3(MARCH_THREADS); kp.kernelParams = p_march;
-    e = cudaGraphAddKernelNode(&n_march, body, &n_emit, 1, &kp);
-    if (e != cudaSuccess) return e;
-    e = cudaGraphInstantiate(&c->loop_exec, c->loop_graph, 0);
-    if (e != cudaSuccess) return e;
+    if ((e = cudaGraphAddKernelNode(&n_march, body, &n_emit, 1, &kp)) != cudaSuccess) return e;
+    if ((e = cudaGraphAddEventRecordNode(&n_ev2, G, &n_while, 1, c->ev[2])) != cudaSuccess) return e;
+    if ((e = set_finalise_params(c, G, &c->loop_finalise, n_ev2, gamma, heat, photons)) != cudaSuccess) return e;
+    double *partial = c->partial, *out = c->scalars + 1;
+    int np = NPARTIAL;
+    void *p_sum[] = {&partial, &np, &out};
+    kp.func = (void *)sum_partials_kernel; kp.gridDim = dim3(1); kp.blockDim = dim3(256); kp.kernelParams = p_sum;
+    if ((e = cudaGraphAddKernelNode(&n_sum, G, &c->loop_finalise, 1, &kp)) != cudaSuccess) return e;
+    if ((e = cudaGraphAddEventRecordNode(&n_ev3, G, &n_sum, 1, c->ev[3])) != cudaSuccess) return e;
+    if ((e = cudaGraphAddMemcpyNode1D(&n_c1, G, &n_ev3, 1, c->h_ds, c->ds, sizeof(DevStats), cudaMemcpyDeviceToHost)) != cudaSuccess) return e;
+    if ((e = cudaGraphAddMemcpyNode1D(&n_c2, G, &n_c1, 1, c->h_scalars, c->scalars, 8 * sizeof(double), cudaMemcpyDeviceToHost)) != cudaSuccess) return e;
+    if ((e = cudaGraphAddMemcpyNode1D(&n_c3, G, &n_c2, 1, c->h_ls, c->ls, sizeof(LoopState), cudaMemcpyDeviceToHost)) != cudaSuccess) return e;
+    if ((e = cudaGraphInstantiate(&c->loop_exec, G, 0)) != cudaSuccess) return e;
     c->loop_args = a;
     c->loop_rank = rank;
     c->loop_world = world;
@@ -480,6 +521,7 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->ev[k]);
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) e = cudaEventCreate(&ctx->tev[k]);
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ls, sizeof(LoopState));
+    if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ls_init, sizeof(LoopState));
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_ds, sizeof(DevStats));
     if (e == cudaSuccess) e = cudaMallocHost(&ctx->h_scalars, 8 * sizeof(double));
     int occ = 0;
@@ -523,6 +565,7 @@ void nyxrt_destroy(nyxrt_ctx *ctx) {
     if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->h_ls) cudaFreeHost(ctx->h_ls);
+    if (ctx->h_ls_init) cudaFreeHost(ctx->h_ls_init);
     if (ctx->h_ds) cudaFreeHost(ctx->h_ds);
     if (ctx->h_scalars) cudaFreeHost(ctx->h_scalars);
     delete ctx;
@@ -640,12 +683,15 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     const long long n_local = ctx->n_cat > ctx->shard_rank ? (ctx->n_cat - ctx->shard_rank + ctx->shard_world - 1) / ctx->shard_world : 0;
     CU(cudaEventRecord(ctx->ev[1], st));
     // ---- ray loop ----
-    CU(cudaMemsetAsync(ctx->acc, 0, ctx->pcell * sizeof(double), st));
-    CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
-    memset(ctx->h_ls, 0, sizeof(LoopState));
-    ctx->h_ls->n_cat = n_local;
-    ctx->h_ls->batch_rays = ctx->batch_rays;
-    CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls, sizeof(LoopState), cudaMemcpyHostToDevice, st));
+    const bool timing = (ctx->p.flags & NYXRT_FLAG_LAUNCH_TIMING) != 0;
+    memset(ctx->h_ls_init, 0, sizeof(LoopState));
+    ctx->h_ls_init->n_cat = n_local;
+    ctx->h_ls_init->batch_rays = ctx->batch_rays;
+    if (timing) {
+        CU(cudaMemsetAsync(ctx->acc, 0, ctx->pcell * sizeof(double), st));
+        CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
+        CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls_init, sizeof(LoopState), cudaMemcpyHostToDevice, st));
+    }
     MarchArgs a;
     memset(&a, 0, sizeof a);
     a.absorber = ctx->absorber;
@@ -683,15 +729,16 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     }
     const int gt = geom_template(ctx->p.geom_mode);
     const int emit_blocks = ctx->sm_count * 4;
-    const bool timing = (ctx->p.flags & NYXRT_FLAG_LAUNCH_TIMING) != 0;
     int chunk = 8;
     long long n_launch = 0;
     if (!timing) {
-        // production: the whole loop is one graph launch; the host synchronises once, after finalise
+        // production: clear, loop, finalise and the copies back are one graph launch; the host synchronises once
         const void *fn = march_fn(gt, ctx->idx64, ctx->g.periodic != 0, lut ? (ctx->d_lut_t ? 2 : 1) : 0);
         if (!ctx->loop_exec || fn != ctx->loop_fn || ctx->loop_rank != ctx->shard_rank || ctx->loop_world != ctx->shard_world ||
             memcmp(&a, &ctx->loop_args, sizeof a) != 0)
-            CU(build_loop_graph(ctx, a, fn, s.L2[0], emit_blocks));
+            CU(build_loop_graph(ctx, a, fn, s.L2[0], emit_blocks, d_gamma, d_heat, d_photons));
+        else if (d_gamma != ctx->loop_gamma || d_heat != ctx->loop_heat || d_photons != ctx->loop_photons)
+            CU(set_finalise_params(ctx, nullptr, &ctx->loop_finalise, nullptr, d_gamma, d_heat, d_photons));
         CU(cudaGraphLaunch(ctx->loop_exec, st));
     }
     for (; timing;) {
@@ -726,16 +773,17 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         if (ctx->h_ls->done) break;
         if (chunk < 256) chunk *= 2;
     }
-    CU(cudaEventRecord(ctx->ev[2], st));
-    // ---- finalise ----
-    const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
-    finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->acc, ctx->absorber, ctx->g.nx, ctx->g.ny, ctx->g.nz, V,
-                                              ctx->p.e_excess_erg, ctx->g.periodic, d_photons, ctx->partial);
-    sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
-    CU(cudaEventRecord(ctx->ev[3], st));
-    CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));
-    CU(cudaMemcpyAsync(ctx->h_scalars, ctx->scalars, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    if (!timing) CU(cudaMemcpyAsync(ctx->h_ls, ctx->ls, sizeof(LoopState), cudaMemcpyDeviceToHost, st));
+    if (timing) {
+        CU(cudaEventRecord(ctx->ev[2], st));
+        // ---- finalise ----
+        const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
+        finalise_kernel<<<NPARTIAL, 256, 0, st>>>(d_gamma, d_heat, ctx->acc, ctx->absorber, ctx->g.nx, ctx->g.ny, ctx->g.nz, V,
+                                                  ctx->p.e_excess_erg, ctx->g.periodic, d_photons, ctx->partial);
+        sum_partials_kernel<<<1, 256, 0, st>>>(ctx->partial, NPARTIAL, ctx->scalars + 1);
+        CU(cudaEventRecord(ctx->ev[3], st));
+        CU(cudaMemcpyAsync(ctx->h_ds, ctx->ds, sizeof(DevStats), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(ctx->h_scalars, ctx->scalars, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    }
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
     if (!timing) {
