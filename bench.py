@@ -57,7 +57,6 @@ def parse():
     ap.add_argument("--graph-loop", action="store_true",
                     help="time the production loop (one CUDA-graph launch per trace; no per-launch events, so the "
                          "roofline's achieved figure then uses the loop time instead of the march launches' own)")
-    ap.add_argument("--window-march", action="store_true", help="experimental march kernel (NYXRT_FLAG_WINDOW_MARCH)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -258,8 +257,6 @@ def main():
     fdt = "f32" if nH.dtype == torch.float32 else "f64"
     params = dict(cfg["params"])
     params["flags"] = 0 if args.graph_loop else nyxrt.FLAG_LAUNCH_TIMING    # per-launch events: what the roofline needs
-    if args.window_march:
-        params["flags"] |= nyxrt.FLAG_WINDOW_MARCH
     tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], params, field_dtype=nH.dtype, max_sources=len(L),
                       batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local,
                       periodic=1 if args.periodic else 0)

@@ -41,7 +41,6 @@ extern "C" {
                                         pair of CUDA events around every march launch (stats ms_march); without it the
                                         loop runs as one CUDA-graph launch (a WHILE node over sched -> emit -> march) and
                                         ms_march is 0.  Same kernels, same results. */
-#define NYXRT_FLAG_WINDOW_MARCH 2    /* experimental march kernel (window.cuh): open box, monochromatic, geom_mode 2 / 3 */
 
 typedef struct nyxrt_ctx nyxrt_ctx;      /* opaque */
 

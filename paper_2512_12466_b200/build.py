@@ -8,7 +8,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "nyxrt.cu")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("nyxrt.cu", "march.cuh", "sources.cuh", "timestep.cuh", "healpix.cuh", "state.cuh", "window.cuh")]
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("nyxrt.cu", "march.cuh", "sources.cuh", "timestep.cuh", "healpix.cuh", "state.cuh")]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "nyxrt.h"))
 LIB = os.path.join(HERE, "libnyxrt.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -16,7 +16,6 @@
 
 #include "../../include/nyxrt.h"
 #include "march.cuh"
-#include "window.cuh"
 #include "sources.cuh"
 #include "timestep.cuh"
 
@@ -84,14 +83,6 @@ struct nyxrt_ctx {
     cudaEvent_t *mev;                      // pairs of events around every march launch
     long long mev_cap;
     cudaStream_t own_stream;
-    // window march (window.cuh): sort buffers of a batch and the blocks' lists of rays alive between two windows
-    uint32_t *wkey_in, *wkey_out, *wval_in, *wval_out;
-    void *wsort_tmp;
-    size_t wsort_bytes;
-    unsigned long long *wl_key;
-    double *wl_tau, *wl_N;
-    int *wl_base;
-    int win_blocks;
     // the ray loop as one CUDA-graph launch: WHILE node over sched -> emit -> march (rebuilt when its arguments change)
     cudaGraph_t loop_graph;
     cudaGraphExec_t loop_exec;
@@ -162,9 +153,9 @@ int effective_levels(const nyxrt_ctx *c) {
 }
 
 // the march's geometry stage runs ahead of its box-exit test: a ray that is leaving may read (never use) up to
-// three planes plus one neighbour offset beyond the halo (the window march: eight cells plus a neighbour); the absorber field carries this many guard cells on
+// three planes plus one neighbour offset beyond the halo; the absorber field carries this many guard cells on
 // both sides, and the cell index type must be able to address them
-long long guard_cells(const nyxrt_grid &g) { return 10 * ((long long)(g.nx + 2) * (g.ny + 2) + (g.nx + 2) + 4); }
+long long guard_cells(const nyxrt_grid &g) { return 4 * ((long long)(g.nx + 2) * (g.ny + 2) + (g.nx + 2) + 4); }
 
 uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, int staging) {
     Bump b{static_cast<char *>(base), 0};
@@ -190,22 +181,6 @@ uint64_t layout(nyxrt_ctx *c, void *base, long long max_sources, long long B, in
     c->pool.s = b.take<double>(total);
     c->pool.tau = b.take<double>(total);
     c->pool.N = b.take<double>(total);
-    {
-        c->wkey_in = b.take<uint32_t>(B);
-        c->wkey_out = b.take<uint32_t>(B);
-        c->wval_in = b.take<uint32_t>(B);
-        c->wval_out = b.take<uint32_t>(B);
-        size_t sb = 0;
-        cub::DeviceRadixSort::SortPairs(nullptr, sb, (uint32_t *)nullptr, (uint32_t *)nullptr, (uint32_t *)nullptr,
-                                        (uint32_t *)nullptr, (int)B);
-        c->wsort_bytes = sb + 256;
-        c->wsort_tmp = b.take<char>(c->wsort_bytes);
-        const long long nl = (long long)c->win_blocks * 2 * WIN_CHUNK;
-        c->wl_key = b.take<unsigned long long>(nl);
-        c->wl_tau = b.take<double>(nl);
-        c->wl_N = b.take<double>(nl);
-        c->wl_base = b.take<int>(nl);
-    }
     SrcBufs &s = c->sb;
     s.pos = b.take<double>(3 * n);
     s.L = b.take<double>(n);
@@ -573,12 +548,6 @@ int nyxrt_create(const nyxrt_grid *grid, const nyxrt_params *params, nyxrt_ctx *
     }
     ctx->sm_count = prop.multiProcessorCount;
     ctx->march_blocks = ctx->sm_count * (occ > 0 ? occ : 1);
-    {
-        int occ_w = 0;
-        cudaFuncSetAttribute(window_march_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_w, window_march_kernel, WIN_THREADS, 0) != cudaSuccess) occ_w = 1;
-        ctx->win_blocks = ctx->sm_count * (occ_w > 0 ? occ_w : 1);
-    }
     *out = ctx;
     return NYXRT_OK;
 }
@@ -762,22 +731,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     const int emit_blocks = ctx->sm_count * 4;
     int chunk = 8;
     long long n_launch = 0;
-    // window march (opt-in, open box, monochromatic, Eq. 7-8 mode, 32-bit indices): host-enqueued loop
-    const bool win = (ctx->p.flags & NYXRT_FLAG_WINDOW_MARCH) != 0 && !ctx->g.periodic && !lut && gt == 3 && !ctx->idx64 &&
-                     ctx->batch_rays < (1ll << 31);
-    int wbits = 1;
-    WinArgs wa;
-    if (win) {
-        const long long groups = (12ll << (2 * (ctx->nlev - 1))) / WIN_PIX + 1;
-        while ((1ll << wbits) <= groups) ++wbits;
-        memset(&wa, 0, sizeof wa);
-        wa.m = a;
-        wa.gkey = ctx->wkey_out;
-        wa.order = ctx->wval_out;
-        wa.lkey = ctx->wl_key; wa.ltau = ctx->wl_tau; wa.lN = ctx->wl_N; wa.lbase = ctx->wl_base;
-        wa.hole_key = 1u << wbits;
-    }
-    if (!timing && !win) {
+    if (!timing) {
         // production: clear, loop, finalise and the copies back are one graph launch; the host synchronises once
         const void *fn = march_fn(gt, ctx->idx64, ctx->g.periodic != 0, lut ? (ctx->d_lut_t ? 2 : 1) : 0);
         if (!ctx->loop_exec || fn != ctx->loop_fn || ctx->loop_rank != ctx->shard_rank || ctx->loop_world != ctx->shard_world ||
@@ -787,12 +741,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
             CU(set_finalise_params(ctx, nullptr, &ctx->loop_finalise, nullptr, d_gamma, d_heat, d_photons));
         CU(cudaGraphLaunch(ctx->loop_exec, st));
     }
-    if (win && !timing) {
-        CU(cudaMemsetAsync(ctx->acc, 0, ctx->pcell * sizeof(double), st));
-        CU(cudaMemsetAsync(ctx->ds, 0, sizeof(DevStats), st));
-        CU(cudaMemcpyAsync(ctx->ls, ctx->h_ls_init, sizeof(LoopState), cudaMemcpyHostToDevice, st));
-    }
-    for (; timing || win;) {
+    for (; timing;) {
         for (int i = 0; i < chunk; ++i) {
             sched_kernel<<<1, 32, 0, st>>>(ctx->ls, ctx->ds, ctx->pool, ctx->nlev, (cudaGraphConditionalHandle)0, 0);
             emit_kernel<<<emit_blocks, 256, 0, st>>>(ctx->ls, ctx->pool, s.L2[0], ctx->shard_rank, ctx->shard_world);
@@ -804,16 +753,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
                 for (long long k = ctx->mev_cap; k < cap; ++k) CU(cudaEventCreate(&ctx->mev[k]));
                 ctx->mev_cap = cap;
             }
-            if (win) {
-                window_keys_kernel<<<ctx->sm_count * 4, 256, 0, st>>>(ctx->ls, ctx->pool, ctx->wkey_in, ctx->wval_in, ctx->batch_rays,
-                                                                      1u << wbits);
-                size_t tb = ctx->wsort_bytes;
-                CU(cub::DeviceRadixSort::SortPairs(ctx->wsort_tmp, tb, ctx->wkey_in, ctx->wkey_out, ctx->wval_in, ctx->wval_out,
-                                                   (int)ctx->batch_rays, 0, wbits + 2, st));
-            }
             CU(cudaEventRecord(ctx->mev[2 * n_launch], st));
-            if (win) window_march_kernel<<<ctx->win_blocks, WIN_THREADS, 0, st>>>(wa);
-            else
             switch (gt) {
                 case 0: launch_march<0, 0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
                 case 1: launch_march<1, 0>(a, ctx->idx64, ctx->g.periodic != 0, ctx->march_blocks, st); break;
@@ -833,7 +773,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         if (ctx->h_ls->done) break;
         if (chunk < 256) chunk *= 2;
     }
-    if (timing || win) {
+    if (timing) {
         CU(cudaEventRecord(ctx->ev[2], st));
         // ---- finalise ----
         const double V = ctx->g.dx_cm * ctx->g.dx_cm * ctx->g.dx_cm;
@@ -846,7 +786,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
     }
     CU(cudaStreamSynchronize(st));
     CU(cudaGetLastError());
-    if (!timing && !win) {
+    if (!timing) {
         if (ctx->h_ls->overflow) return fail(ctx, NYXRT_EOVERFLOW, "trace: ray pool overflow at level %d", ctx->h_ls->level + 1);
         n_launch = (long long)ctx->h_ls->iterations + 1;                 // rounds of the WHILE body (the last one is empty)
     }
@@ -876,7 +816,7 @@ static int run_trace(nyxrt_ctx *ctx, double *d_gamma, double *d_heat, double *d_
         cudaEventElapsedTime(&hs->ms_total, ctx->ev[0], ctx->ev[3]);
         double ms = 0.0;
         const long long live = (long long)ctx->h_ls->iterations;       // launches that had a batch
-        for (long long k = 0; (timing || win) && k < n_launch && k < live; ++k) {
+        for (long long k = 0; timing && k < n_launch && k < live; ++k) {
             float t = 0.f;
             cudaEventElapsedTime(&t, ctx->mev[2 * k], ctx->mev[2 * k + 1]);
             ms += t;

@@ -13,7 +13,6 @@ from . import build as _build
 MAXLEV = 16
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EOVERFLOW = 0, -1, -2, -3, -4, -5
 FLAG_LAUNCH_TIMING = 1
-FLAG_WINDOW_MARCH = 2
 _ERRNAME = {EINVAL: "NYXRT_EINVAL", ESTATE: "NYXRT_ESTATE", ENOMEM: "NYXRT_ENOMEM", ECUDA: "NYXRT_ECUDA",
             EOVERFLOW: "NYXRT_EOVERFLOW"}
 

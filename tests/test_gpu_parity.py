@@ -247,28 +247,3 @@ def test_graph_loop_and_profiling_loop_are_the_same_step(O):
     finally:
         tr.close()
     assert seg == [sg.segments] * 4 and s0 + s1 == sg.segments and 0 < s0 < sg.segments
-
-
-@pytest.mark.parametrize("case", ["config3", "config4_merge", "config5_f32", "thin_long", "config2", "config1"])
-def test_window_march_kernel(O, case):
-    """NYXRT_FLAG_WINDOW_MARCH: the march in windows of a geometry shared by all rays of a pixel group (window.cuh)
-    against the oracle, by the same rule: counters exact, rates to 1e-9."""
-    from paper_2512_12466_b200 import nyxrt
-    fl = dict(flags=nyxrt.FLAG_WINDOW_MARCH)
-    if case == "config3":
-        for batch in (0, 4096, 352):
-            both(O, synth.make(3, n=64, n_src=400), params=fl, batch_rays=batch)
-    elif case == "config4_merge":
-        worst, rg, ro = both(O, synth.make(4, n=64, n_src=3000), params=fl, batch_rays=16384)
-        assert rg[2].n_src_merged < rg[2].n_src_dedup
-    elif case == "config5_f32":
-        both(O, synth.make(5, n=80, n_src=4000), params=fl, batch_rays=20000)
-    elif case == "thin_long":
-        cfg = synth.make(3, n=96, n_src=12)
-        cfg["xHI"] = cfg["xHI"] * 1e-3
-        worst, rg, ro = both(O, cfg, params=fl, batch_rays=8192)
-        assert sum(rg[2].exited) > 1000 and rg[2].spawned[6] > 0
-    elif case == "config2":
-        both(O, synth.make(2, n=48), params=fl)
-    else:
-        both(O, synth.make(1), params=fl)
