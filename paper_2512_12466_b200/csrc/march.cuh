@@ -113,8 +113,8 @@ __global__ void emit_kernel(const LoopState *ls, RayPool pool, const double *cat
 
 // ---------------------------------------------------------------------------------------------------
 // pm = e^-x - 1 (minus the absorbed fraction) and left = e^-x for x >= 0 (not DEC: the tolerance is 1e-9,
-// DESIGN.md "Tolerances").  Thin cells (x < 2^-7, the ionised phase) take a short series; otherwise
-// x = k ln2 + r with |r| <= ln2/2; e^-r - 1 = u + u^2 q(u), u = -r, by its Taylor series through u^11
+// DESIGN.md "Tolerances").  One branch-free routine for thin and thick cells (they sit side by side in every warp):
+// x = k ln2 + r with |r| <= ln2/2 (k = 0 for a thin cell); e^-r - 1 = u + u^2 q(u), u = -r, by its Taylor series through u^11
 // (remainder < 2e-14 relative); left = 2^-k (1 + p), pm = 2^-k p + (2^-k - 1): e^-x - 1 keeps full relative
 // accuracy where 1 - exp(-x) would not.  Coefficients sit in constant memory so that they are
 // operands, not re-materialised immediates.
