@@ -6,8 +6,10 @@ sources, merging on), per GPU.  See DESIGN.md "Measurement".
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--n-src N]
 
 Prints ONE JSON line (rank 0).  metric = ray-cell segments per second over the whole RT step.
-N > 1 (torchrun): the path does not shard on the graded configuration ("replicas only", DESIGN.md
-"Multi-GPU"): every rank runs the same step on its own GPU; value = N * segments / max-over-ranks time.
+N > 1 (torchrun): the step is sharded by source: every rank builds the whole catalogue,
+traces the entries rank, rank + N, ..., the photon grids are all-reduced once and finalised; value = all ranks'
+segments / max-over-ranks time ("scaling": "strong").  `--replicas`: every rank runs the whole step on its own GPU
+instead (redundant work; value = N * segments / max-over-ranks time, "scaling": "weak").
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 import argparse

@@ -1,6 +1,7 @@
-"""Host logic of bench.py's N > 1 path ("replicas only": no data-path collective; the only exchange is the
-max-over-ranks of the timing), run as two gloo ranks on the CPU; and the --impl reference rule that only
-rank 0 works."""
+"""Host logic of bench.py's N > 1 paths (the max-over-ranks of the timing; the sum of the ranks' own segments in
+the source-sharded mode; the --replicas rate), run as two gloo ranks on the CPU; and the --impl reference rule
+that only rank 0 works.  The data path of the sharded mode (one all-reduce of the photon grid) is exercised
+across two processes on a GPU in tests/test_gpu_multiproc.py."""
 import os
 import subprocess
 import sys
