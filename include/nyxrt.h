@@ -204,6 +204,46 @@ int nyxrt_trace_photons(nyxrt_ctx *ctx, double *d_photons, nyxrt_stats *h_stats,
 int nyxrt_finalise(nyxrt_ctx *ctx, const double *d_photons, double *d_gamma_HI, double *d_heat, double *h_absorbed,
                    void *cuda_stream);
 
+/* nyxrt_finalise for callers that must not allocate device memory: no context, no workspace, no cudaMalloc /
+ * cudaFree / cudaMallocHost and no library routine that allocates, on any call.
+ *
+ * Why it exists.  The library is meant to run inside a host code that owns the GPU's memory: Nyx's AMReX arena
+ * (or, under the Python binding, PyTorch's caching allocator) has usually taken nearly all of it, so a cudaMalloc
+ * made from here can fail while the host code still has free blocks, and every cudaMalloc / cudaFree stalls all
+ * streams of the device.  The other entry points need a context (a few small allocations in nyxrt_create) and a
+ * workspace the caller allocates.  A caller that can afford neither -- e.g. a rank that only turns the all-reduced
+ * photon grid of a source-sharded step into rates, or a diagnostic run between two kernels of a time step -- calls
+ * this instead.
+ *
+ * What it computes (Eq. 1 with V_box; heating: reading H1), from device pointers,
+ * all [nz][ny][nx], x fastest:
+ *   d_nH, d_xHI     in   total hydrogen density [cm^-3] and NEUTRAL fraction, fp64 (field_dtype 0) or fp32 (1)
+ *   d_photons       in   photons absorbed per cell per second (nyxrt_trace_photons, summed over shards), fp64
+ *   d_gamma_HI      out  photons / (n_H x_HI dx_cm^3), exactly 0 where photons == 0; same bits as nyxrt_finalise
+ *   d_heat          out  e_excess_erg * photons / dx_cm^3; may be NULL
+ *   d_absorbed      out  one double: sum of d_photons (row sums in x order, rows in a fixed order: the same bits on
+ *                        every call, equal to nyxrt_finalise's total up to the rounding of a different but also
+ *                        fixed summation order); may be NULL
+ * All buffers stay the caller's; nothing is retained.  The two kernels are enqueued on `cuda_stream` on `device`
+ * (made current, as the other entry points do); the call does not synchronise.
+ *
+ * The scratch (one partial sum per row) is a fixed array inside the library: NYXRT_STATIC_MAX_ROWS doubles (8 MiB)
+ * on every GPU that loads libnyxrt.so, for the life of the process.  Hence:
+ *   - ny * nz > NYXRT_STATIC_MAX_ROWS (more rows than the 1024^3 grid of config 5) -> NYXRT_ENOMEM, nothing enqueued;
+ *   - every call in the process shares the array, which still holds the previous call's partials.  No part of it
+ *     needs clearing (a call reads only the ny * nz entries it has just written), but two calls that run on the
+ *     same GPU at the same time -- two streams, or two host threads -- corrupt each other's d_absorbed.  Put them
+ *     on one stream or order them with events;
+ *   - the first call that names a device looks up the array's address on that device
+ *     (cudaGetSymbolAddress); make that first call before any stream capture begins.
+ * errbuf (may be NULL) receives the message of a failed call, truncated to errbuf_len bytes.
+ * Errors: EINVAL (sizes, dtype, dx_cm <= 0, NULL, device ordinal outside 0..63), ENOMEM (grid beyond the scratch), ECUDA. */
+#define NYXRT_STATIC_MAX_ROWS (1 << 20)
+int nyxrt_finalise_static(int32_t device, int32_t nx, int32_t ny, int32_t nz, int32_t field_dtype, double dx_cm,
+                          double e_excess_erg, const void *d_nH, const void *d_xHI, const double *d_photons,
+                          double *d_gamma_HI, double *d_heat, double *d_absorbed, void *cuda_stream, char *errbuf,
+                          int64_t errbuf_len);
+
 /* The (deduplicated, merged, sorted) catalogue the last nyxrt_trace used: host
  * pointers with room for `cap` entries; cell_ijk is [cap][3]; radius is the bubble radius in cells
  * (0 when merging was off).  Any of the three arrays may be NULL.  *n_out = catalogue length even

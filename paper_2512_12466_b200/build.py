@@ -8,7 +8,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "nyxrt.cu")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("nyxrt.cu", "march.cuh", "sources.cuh", "timestep.cuh", "healpix.cuh", "state.cuh")]
+SRC_STATIC = os.path.join(HERE, "csrc", "finalise_static.cu")      # nyxrt_finalise_static: its own translation unit
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("nyxrt.cu", "finalise_static.cu", "march.cuh", "sources.cuh", "timestep.cuh", "healpix.cuh", "state.cuh")]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "nyxrt.h"))
 LIB = os.path.join(HERE, "libnyxrt.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -27,7 +28,7 @@ def build(force=False, verbose=False):
     if not force and not stale():
         return LIB
     tmp = LIB + ".%d.tmp" % os.getpid()
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, SRC]
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, SRC, SRC_STATIC]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

@@ -13,6 +13,7 @@ from . import build as _build
 MAXLEV = 16
 OK, EINVAL, ESTATE, ENOMEM, ECUDA, EOVERFLOW = 0, -1, -2, -3, -4, -5
 FLAG_LAUNCH_TIMING = 1
+STATIC_MAX_ROWS = 1 << 20      # NYXRT_STATIC_MAX_ROWS: largest ny * nz nyxrt_finalise_static accepts
 _ERRNAME = {EINVAL: "NYXRT_EINVAL", ESTATE: "NYXRT_ESTATE", ENOMEM: "NYXRT_ENOMEM", ECUDA: "NYXRT_ECUDA",
             EOVERFLOW: "NYXRT_EOVERFLOW"}
 
@@ -76,7 +77,7 @@ EXPORTS = ["nyxrt_create", "nyxrt_workspace_bytes", "nyxrt_set_workspace", "nyxr
            "nyxrt_destroy", "nyxrt_version", "nyxrt_sizeof_grid", "nyxrt_sizeof_params", "nyxrt_sizeof_stats",
            "nyxrt_timestep", "nyxrt_sizeof_ode", "nyxrt_sizeof_tstats", "nyxrt_set_shard", "nyxrt_trace_photons",
            "nyxrt_finalise", "nyxrt_spectrum_nodes", "nyxrt_spectrum_node_tau", "nyxrt_set_spectrum",
-           "nyxrt_blackbody_table", "nyxrt_set_spectrum_thin", "nyxrt_blackbody_thin_table"]
+           "nyxrt_blackbody_table", "nyxrt_set_spectrum_thin", "nyxrt_blackbody_thin_table", "nyxrt_finalise_static"]
 
 _lib = None
 
@@ -239,6 +240,30 @@ def nyxrt_finalise(ctx, photons, gamma, heat=None, stream=None):
                                      C.c_void_p(heat.data_ptr()) if heat is not None else None, C.byref(absorbed),
                                      _stream_ptr(stream)))
     return absorbed.value
+
+
+def nyxrt_finalise_static(nH, xHI, photons, gamma, dx_cm, e_excess_erg=0.0, heat=None, absorbed=None, stream=None):
+    """nyxrt_finalise without a context or workspace, for code that must not allocate device memory (the host
+    application's arena or torch's caching allocator owns the GPU, and cudaMalloc stalls every stream): the scratch
+    is a fixed 8 MiB array inside the library, so grids are limited to ny * nz <= STATIC_MAX_ROWS rows and calls that
+    overlap on one GPU race on it.  All tensors are the caller's CUDA tensors of shape [nz][ny][nx]; `absorbed` is a
+    1-element fp64 CUDA tensor that receives the sum of `photons` (or None).  Enqueues on `stream`, does not
+    synchronise.  This wrapper only marshals: it creates no tensor."""
+    for t in (photons, gamma) + tuple(x for x in (heat, absorbed) if x is not None):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    assert nH.is_cuda and xHI.is_cuda and nH.is_contiguous() and xHI.is_contiguous() and nH.dtype == xHI.dtype
+    assert nH.dtype in (torch.float32, torch.float64) and nH.dim() == 3
+    assert nH.shape == xHI.shape == photons.shape == gamma.shape and (heat is None or heat.shape == nH.shape)
+    nz, ny, nx = nH.shape
+    err = C.create_string_buffer(256)
+    rc = lib().nyxrt_finalise_static(
+        C.c_int32(nH.device.index or 0), C.c_int32(nx), C.c_int32(ny), C.c_int32(nz),
+        C.c_int32(1 if nH.dtype == torch.float32 else 0), C.c_double(dx_cm), C.c_double(e_excess_erg),
+        C.c_void_p(nH.data_ptr()), C.c_void_p(xHI.data_ptr()), C.c_void_p(photons.data_ptr()),
+        C.c_void_p(gamma.data_ptr()), C.c_void_p(heat.data_ptr()) if heat is not None else None,
+        C.c_void_p(absorbed.data_ptr()) if absorbed is not None else None, _stream_ptr(stream), err, C.c_int64(len(err)))
+    if rc != OK:
+        raise NyxrtError(rc, err.value.decode())
 
 
 def nyxrt_timestep(ctx, ode, nH, xHI_begin, xHI_end, xHI_avg, gamma, heat=None, stream=None):
