@@ -163,7 +163,9 @@ int nyxrt_trace(nyxrt_ctx *ctx, double *d_gamma_HI, double *d_heat, nyxrt_stats 
  *                             (the default: Q = 1 - e^-tau evaluated in the kernel).  Needs geom_mode 2 or 3.
  *                             Choose tau_max (nyxrt_params) for the spectrum: hard photons outlive tau_0 = ln 1e8.
  *   nyxrt_blackbody_table     fills h_q with Q of a black body of temperature t_eff_K above 13.6 eV (R39)
- * Heating stays e_excess_erg per absorbed photon (H1).  Errors: EINVAL, ECUDA. */
+ * Heating stays e_excess_erg per absorbed photon (H1).  A call that fails changes nothing: the Q table and the thin
+ * table set before stay active (a successful call with a new Q table, or h_q = NULL, drops the thin table).
+ * Errors: EINVAL, ECUDA. */
 int nyxrt_spectrum_nodes(int32_t e_lo, int32_t e_hi, int32_t m, int64_t *n);
 int nyxrt_spectrum_node_tau(int32_t e_lo, int32_t m, int64_t k, double *tau);
 int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, const double *h_q, int64_t n);
@@ -178,7 +180,8 @@ int nyxrt_blackbody_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m,
  * interpolated Q values; the photons a ray carries are then counted down segment by segment (the two forms do not
  * telescope into each other).  The neighbour's share of Eq. 6 / 8 is (1 - f_c) of the absorbed photons either way.
  *   nyxrt_set_spectrum_thin    h_t: host array of n values >= 0, copied (h_t = NULL: thin table off).  A later
- *                              nyxrt_set_spectrum drops it.  Errors: EINVAL, ESTATE (no Q table), ECUDA.
+ *                              successful nyxrt_set_spectrum drops it; a failed call of either function leaves the
+ *                              tables as they were.  Errors: EINVAL, ESTATE (no Q table), ECUDA.
  *   nyxrt_blackbody_thin_table T of a black body of temperature t_eff_K above 13.6 eV on the given nodes. */
 int nyxrt_set_spectrum_thin(nyxrt_ctx *ctx, const double *h_t, int64_t n, double tau_thin);
 int nyxrt_blackbody_thin_table(double t_eff_K, int32_t e_lo, int32_t e_hi, int32_t m, double *h_t, int64_t n);

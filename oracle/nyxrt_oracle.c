@@ -423,15 +423,21 @@ double orc_spectrum_node_tau(int e_lo, int m, int64_t k) {
 }
 
 int orc_set_spectrum(int e_lo, int e_hi, int m, const double *q, int64_t n) {
+    if (q) {                                                            /* a rejected call leaves both tables as they were */
+        if (e_lo < -1000 || e_hi > 1000 || e_hi <= e_lo || m < 0 || m > 20 || n != orc_spectrum_nodes(e_lo, e_hi, m))
+            return ORC_EINVAL;
+    }
+    double *copy = NULL;
+    if (q) {
+        copy = malloc((size_t)n * sizeof *q);
+        if (!copy) return ORC_ENOMEM;
+        memcpy(copy, q, (size_t)n * sizeof *q);
+    }
     free(g_lut.q);
-    free(g_lut.t);
+    free(g_lut.t);                                                      /* a new Q table drops the thin table */
     memset(&g_lut, 0, sizeof g_lut);
     if (!q) return ORC_OK;                                              /* back to monochromatic */
-    if (e_lo < -1000 || e_hi > 1000 || e_hi <= e_lo || m < 0 || m > 20 || n != orc_spectrum_nodes(e_lo, e_hi, m))
-        return ORC_EINVAL;
-    g_lut.q = malloc((size_t)n * sizeof *q);
-    if (!g_lut.q) return ORC_ENOMEM;
-    memcpy(g_lut.q, q, (size_t)n * sizeof *q);
+    g_lut.q = copy;
     g_lut.on = 1; g_lut.e_lo = e_lo; g_lut.e_hi = e_hi; g_lut.m = m; g_lut.n = n;
     return ORC_OK;
 }
@@ -461,15 +467,16 @@ double orc_spectrum_q(double tau) {
    being read off Q(tau_0) [R42].  The neighbour's share (Eq. 6 / 8) is (1 - f_c) of whatever the segment absorbed,
    in photons: no quotient of absorber densities is formed, which is the part the footnote calls "not applicable". */
 int orc_set_spectrum_thin(const double *t, int64_t n, double tau_thin) {
+    double *copy = NULL;
+    if (t) {                                                            /* a rejected call leaves the thin table in place */
+        if (!g_lut.on || n != g_lut.n || !(tau_thin >= 0.0)) return ORC_EINVAL;
+        copy = malloc((size_t)n * sizeof *t);
+        if (!copy) return ORC_ENOMEM;
+        memcpy(copy, t, (size_t)n * sizeof *t);
+    }
     free(g_lut.t);
-    g_lut.t = NULL;
-    g_lut.tau_thin = 0.0;
-    if (!t) return ORC_OK;
-    if (!g_lut.on || n != g_lut.n || !(tau_thin >= 0.0)) return ORC_EINVAL;
-    g_lut.t = malloc((size_t)n * sizeof *t);
-    if (!g_lut.t) return ORC_ENOMEM;
-    memcpy(g_lut.t, t, (size_t)n * sizeof *t);
-    g_lut.tau_thin = tau_thin;
+    g_lut.t = copy;
+    g_lut.tau_thin = t ? tau_thin : 0.0;
     return ORC_OK;
 }
 

@@ -851,13 +851,14 @@ int nyxrt_spectrum_node_tau(int32_t e_lo, int32_t m, int64_t k, double *tau) {
 int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, const double *h_q, int64_t n) {
     if (!ctx) return NYXRT_EINVAL;
     CU(cudaSetDevice(ctx->g.device));
-    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);                              // a new Q table drops the thin table
-    ctx->d_lut_t = nullptr;
-    if (!h_q) {                                                            // back to monochromatic
+    if (!h_q) {                                                            // back to monochromatic: both tables go
+        if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
+        ctx->d_lut_t = nullptr;
         if (ctx->d_lut) cudaFree(ctx->d_lut);
         ctx->d_lut = nullptr;
         return NYXRT_OK;
     }
+    // a rejected call changes nothing: both tables stay as they were until the new Q table is on the device
     int64_t need = 0;
     if (nyxrt_spectrum_nodes(e_lo, e_hi, m, &need) != NYXRT_OK || n != need)
         return fail(ctx, NYXRT_EINVAL, "set_spectrum: bad table geometry or length");
@@ -866,8 +867,6 @@ int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, co
     for (int64_t k = 0; k < n; ++k)
         if (!(h_q[k] >= 0.0) || !(h_q[k] <= 1.0) || (k > 0 && h_q[k] < h_q[k - 1]))
             return fail(ctx, NYXRT_EINVAL, "set_spectrum: Q must be non-decreasing within [0, 1]");
-    if (ctx->d_lut) cudaFree(ctx->d_lut);
-    ctx->d_lut = nullptr;
     double *d = nullptr;
     CU(cudaMalloc(&d, n * sizeof(double)));
     const cudaError_t ce = cudaMemcpy(d, h_q, n * sizeof(double), cudaMemcpyHostToDevice);
@@ -875,6 +874,9 @@ int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, co
         cudaFree(d);
         return fail(ctx, NYXRT_ECUDA, "set_spectrum: copy failed: %s", cudaGetErrorString(ce));
     }
+    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);                              // a new Q table drops the thin table
+    ctx->d_lut_t = nullptr;
+    if (ctx->d_lut) cudaFree(ctx->d_lut);
     ctx->d_lut = d;
     ctx->lut_e_lo = e_lo; ctx->lut_e_hi = e_hi; ctx->lut_m = m; ctx->lut_n = n;
     ctx->lut_first = h_q[0];
@@ -885,9 +887,12 @@ int nyxrt_set_spectrum(nyxrt_ctx *ctx, int32_t e_lo, int32_t e_hi, int32_t m, co
 int nyxrt_set_spectrum_thin(nyxrt_ctx *ctx, const double *h_t, int64_t n, double tau_thin) {
     if (!ctx) return NYXRT_EINVAL;
     CU(cudaSetDevice(ctx->g.device));
-    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
-    ctx->d_lut_t = nullptr;
-    if (!h_t) return NYXRT_OK;
+    if (!h_t) {                                                            // thin table off
+        if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
+        ctx->d_lut_t = nullptr;
+        return NYXRT_OK;
+    }
+    // as in set_spectrum: a rejected call leaves the thin table that was set before in place
     if (!ctx->d_lut) return fail(ctx, NYXRT_ESTATE, "set_spectrum_thin: set the Q table first");
     if (n != ctx->lut_n || !(tau_thin >= 0.0)) return fail(ctx, NYXRT_EINVAL, "set_spectrum_thin: bad length or threshold");
     for (int64_t k = 0; k < n; ++k)
@@ -899,6 +904,7 @@ int nyxrt_set_spectrum_thin(nyxrt_ctx *ctx, const double *h_t, int64_t n, double
         cudaFree(d);
         return fail(ctx, NYXRT_ECUDA, "set_spectrum_thin: copy failed: %s", cudaGetErrorString(ce));
     }
+    if (ctx->d_lut_t) cudaFree(ctx->d_lut_t);
     ctx->d_lut_t = d;
     ctx->lut_t_first = h_t[0];
     ctx->lut_t_last = h_t[n - 1];

@@ -125,6 +125,42 @@ def test_set_spectrum_drops_the_thin_table_and_errors():
         tr.close()
 
 
+def test_a_rejected_set_spectrum_leaves_both_tables_in_place(tabs):
+    """A failed nyxrt_set_spectrum / nyxrt_set_spectrum_thin (bad length, non-monotone Q, negative T) must change
+    nothing: the next trace still uses the Q table AND the thin table set before.  The thin table here is half the
+    true one, so that a silently dropped table would move Gamma by tens of per cent, far beyond the run-to-run
+    difference of the deposits' summation order."""
+    cfg = synth.make(4, n=32, n_src=60)
+    p = dict(cfg["params"], tau_max=60.0)
+    tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], p, field_dtype=cfg["nH"].dtype, max_sources=60)
+    try:
+        tr.set_fields(cfg["nH"].cuda().contiguous(), cfg["xHI"].cuda().contiguous())
+        tr.set_sources(cfg["src_pos"].numpy(), cfg["src_L"].numpy())
+        tr.set_spectrum(E_LO, E_HI, M, tabs[0])
+        g_one = tr.trace()[0].clone()                                           # Q table alone
+        tr.set_spectrum_thin(0.5 * tabs[1], 2.0 ** -4)
+        g_two = tr.trace()[0].clone()                                           # with the (halved) thin table
+        assert float(((g_two - g_one).abs() > 0.1 * g_one).double().mean()) > 0.1
+        bad_q = tabs[0].copy()
+        bad_q[5] = bad_q[4] - 1e-3
+        for call in (lambda: tr.set_spectrum(E_LO, E_HI, M, tabs[0][:-1]),      # wrong length
+                     lambda: tr.set_spectrum(E_LO, E_HI + 1, M, tabs[0]),       # geometry does not match the length
+                     lambda: tr.set_spectrum(E_LO, E_HI, M, bad_q),             # not monotone
+                     lambda: tr.set_spectrum_thin(tabs[1][:-1], 2.0 ** -4),
+                     lambda: tr.set_spectrum_thin(-tabs[1], 2.0 ** -4),
+                     lambda: tr.set_spectrum_thin(tabs[1], -1.0)):
+            with pytest.raises(nyxrt.NyxrtError) as e:
+                call()
+            assert e.value.code == nyxrt.EINVAL
+            g = tr.trace()[0]
+            assert bool(((g - g_two).abs() <= 1e-9 * g_two + 1e-30).all())
+        tr.set_spectrum(E_LO, E_HI, M, tabs[0])                                 # a successful one does drop the thin table
+        g = tr.trace()[0]
+        assert bool(((g - g_one).abs() <= 1e-9 * g_one + 1e-30).all())
+    finally:
+        tr.close()
+
+
 def test_timestep_with_both_tables(O, tabs):
     """The RT timestep on top of the two-table flux: the paper's full update, Stroemgren test A."""
     MYR = 3.1557e13

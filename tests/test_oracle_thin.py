@@ -165,3 +165,17 @@ def test_thin_limit_rate(O, tables, mono_after):
         m = (r >= lo) & (r < hi)
         expect = np.mean(sig * O.spectrum_t(k * 0.5 * (lo + hi)) * L / (4 * math.pi * (r[m] * dx) ** 2))
         assert abs(gam[m].mean() - expect) < 0.05 * expect
+
+
+def test_a_rejected_call_leaves_the_oracles_tables_in_place(O, tables, mono_after):
+    """Host logic, no arithmetic: orc_set_spectrum / orc_set_spectrum_thin check their arguments before they touch
+    the tables (the C ABI's rule, include/nyxrt.h), so a failed call changes neither lookup."""
+    q, t = tables
+    O.set_spectrum(E_LO, E_HI, M, q)
+    O.set_spectrum_thin(t, 2.0 ** -8)
+    q_at, t_at = O.spectrum_q(0.37), O.spectrum_t(0.37)
+    for call in (lambda: O.set_spectrum(E_LO, E_HI, M, q[:-1]), lambda: O.set_spectrum(E_LO, E_HI + 1, M, q),
+                 lambda: O.set_spectrum_thin(t[:-1], 2.0 ** -8), lambda: O.set_spectrum_thin(t, -1.0)):
+        with pytest.raises(Exception):
+            call()
+        assert O.spectrum_q(0.37) == q_at and O.spectrum_t(0.37) == t_at
