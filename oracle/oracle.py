@@ -425,38 +425,78 @@ def step_parallel(g, p, nH, xHI, pos, L, n_proc, want_heat=True, chunk=4):
     chunks = [(a, min(n_cat, a + chunk)) for a in range(0, n_cat, chunk)]
     shape = (g.nz, g.ny, g.nx)
     nbytes = int(np.prod(shape)) * 8
+    # The workers' partial grids live in /dev/shm: never ask for more of it than is free (a worker that touches
+    # a page the tmpfs cannot back dies of SIGBUS), and say so instead of failing half-way.
+    import shutil
+    per_proc = nbytes * (2 if want_heat else 1)
+    try:
+        shm_free = shutil.disk_usage("/dev/shm").free
+    except OSError:
+        shm_free = None
+    if shm_free is not None:
+        fit = int(0.9 * shm_free // per_proc)
+        if fit < 1:
+            raise MemoryError("step_parallel: /dev/shm has %.1f GB free, one worker's grids need %.1f GB"
+                              % (shm_free / 1e9, per_proc / 1e9))
+        n_proc = min(n_proc, fit)
+    # fork: the children inherit the fields and the catalogue without a copy and never touch CUDA or threads of the
+    # parent (they only run the single-threaded C oracle), which is what makes forking a process that has
+    # initialised CUDA safe here.
     ctx = mp.get_context("fork")
     counter = ctx.Value(C.c_int64, 0)
     shms, procs, conns, gam_parts, heat_parts = [], [], [], [], []
-    for _ in range(n_proc):
-        pair = [shared_memory.SharedMemory(create=True, size=nbytes) for _ in range(2 if want_heat else 1)]
-        shms += pair
-        gam_parts.append(np.ndarray(shape, np.float64, buffer=pair[0].buf))
-        if want_heat:
-            heat_parts.append(np.ndarray(shape, np.float64, buffer=pair[1].buf))
-        rx, tx = ctx.Pipe(duplex=False)
-        pr = ctx.Process(target=_worker, args=(g, p, nH, xHI, cat, chunks, counter, [s.name for s in pair], shape,
-                                               want_heat, tx))
-        pr.start()
-        tx.close()
-        procs.append(pr)
-        conns.append(rx)
     total = Stats()
     cpu = 0.0
-    for pr, rx in zip(procs, conns):
-        raw, secs = rx.recv()
-        pr.join()
-        if pr.exitcode != 0:
-            raise RuntimeError("oracle worker failed")
-        st = Stats.from_buffer_copy(raw)
-        cpu += secs
-        for name, _ in Stats._fields_:
-            v = getattr(st, name)
-            if hasattr(v, "__len__"):
-                t = getattr(total, name)
-                for l in range(len(v)):
-                    t[l] += v[l]
-            else:
-                setattr(total, name, getattr(total, name) + v)
+    try:
+        for _ in range(n_proc):
+            pair = []
+            for _k in range(2 if want_heat else 1):
+                pair.append(shared_memory.SharedMemory(create=True, size=nbytes))
+                shms.append(pair[-1])
+            gam_parts.append(np.ndarray(shape, np.float64, buffer=pair[0].buf))
+            if want_heat:
+                heat_parts.append(np.ndarray(shape, np.float64, buffer=pair[1].buf))
+            rx, tx = ctx.Pipe(duplex=False)
+            pr = ctx.Process(target=_worker, args=(g, p, nH, xHI, cat, chunks, counter, [s.name for s in pair], shape,
+                                                   want_heat, tx))
+            pr.start()
+            tx.close()
+            procs.append(pr)
+            conns.append(rx)
+        for pr, rx in zip(procs, conns):
+            try:
+                raw, secs = rx.recv()
+            except EOFError:
+                pr.join()
+                raise RuntimeError("oracle worker died (exit code %s) before it reported" % pr.exitcode)
+            pr.join()
+            if pr.exitcode != 0:
+                raise RuntimeError("oracle worker failed (exit code %s)" % pr.exitcode)
+            st = Stats.from_buffer_copy(raw)
+            cpu += secs
+            for name, _ in Stats._fields_:
+                v = getattr(st, name)
+                if hasattr(v, "__len__"):
+                    t = getattr(total, name)
+                    for l in range(len(v)):
+                        t[l] += v[l]
+                else:
+                    setattr(total, name, getattr(total, name) + v)
+    except BaseException:
+        # no orphans and no leaked segments: stop every worker, then give the shared memory back
+        for pr in procs:
+            if pr.is_alive():
+                pr.terminate()
+        for pr in procs:
+            pr.join()
+        gam_parts.clear()
+        heat_parts.clear()
+        for s_ in shms:
+            try:
+                s_.close()
+                s_.unlink()
+            except (OSError, BufferError):
+                pass
+        raise
     total.n_src_in, total.n_src_dedup, total.n_src_merged = st0.n_src_in, st0.n_src_dedup, st0.n_src_merged
     return OracleSum(total, gam_parts, heat_parts, shms, cpu, n_proc), cat
