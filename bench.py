@@ -6,6 +6,12 @@ sources, merging on), per GPU.  See DESIGN.md "Measurement".
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5] [--n-src N]
 
 Prints ONE JSON line (rank 0).  metric = ray-cell segments per second over the whole RT step.
+`value`, `ms_per_step` and `e2e` time the PRODUCTION path: the ray loop as one CUDA-graph launch per trace.  The
+roofline needs the march launches' own durations, which that loop cannot give, so after the timed region
+`--profile-steps` extra step(s) (default 1) run through the host-enqueued loop with a CUDA-event pair around every
+march launch (NYXRT_FLAG_LAUNCH_TIMING; same kernels, same results) and are reported under `profiling_pass`.
+`roofline` is the march kernel against the fp64-pipe roof (bound "alu"; the kernel is issue-bound, not HBM-bound),
+with the issue roof and the three HBM figures (contract bytes, counted bytes, DRAM bytes measured by ncu) beside it.
 N > 1 (torchrun): the step is sharded by source: every rank builds the whole catalogue,
 traces the entries rank, rank + N, ..., the photon grids are all-reduced once and finalised; value = all ranks'
 segments / max-over-ranks time ("scaling": "strong").  `--replicas`: every rank runs the whole step on its own GPU
@@ -28,12 +34,36 @@ ALGO_BYTES_PER_SEGMENT = {"f32": 48, "f64": 64}     # 4 field lo
 # cell, and the same again for each neighbour deposit the library counted (stats.neighbour_deposits)
 ALGO_BYTES_CELL = {"f32": 24, "f64": 32}
 METRIC = "ray_cell_segments_per_s"
-# Secondary (issue) roof of the march kernel: one ray-cell costs 230 executed warp
-# instructions of which 76 are fp64 (profiles/r1_v12_march_config5.md); an fp64 warp instruction holds the
-# sub-partition's fp64 pipe for two cycles while other instructions issue, so a warp-cell takes
-# max(230 issue slots, 2 x 76 fp64-pipe cycles) = 230 cycles of a scheduler.
-ISSUE_CYCLES_PER_WARP_CELL = 230
+# The march kernel's two ALU roofs come from the executed-instruction counts of the
+# shipping kernel in profiles/march_instr.csv (last row; profiles/march_instr.md says how they were taken), not
+# from a constant here:
+#   fp64 pipe: a warp-level fp64 instruction occupies its sub-partition's fp64 pipe for 2 cycles (16 lanes per clock),
+#              so a warp-cell costs 2 x fp64_inst_per_warp_cell cycles of a scheduler whatever else issues beside it;
+#   issue:     one warp instruction per scheduler per cycle: inst_per_warp_cell cycles.
+# segments/s at a roof = SMs x 4 schedulers x SM clock x 32 lanes / cycles per warp-cell (all lanes busy, no stall).
 SM_COUNT, SCHEDULERS_PER_SM, LANES = 148, 4, 32
+FP64_PIPE_CYCLES_PER_WARP_INST = 2
+
+
+def march_instruction_counts(path=None):
+    """(inst_per_warp_cell, fp64_inst_per_warp_cell, profile name) of the shipping march kernel."""
+    import csv
+    path = path or os.path.join(ROOT, "profiles", "march_instr.csv")
+    with open(path, newline="") as f:
+        rows = list(csv.DictReader(f))
+    r = rows[-1]
+    return float(r["inst_per_warp_cell"]), float(r["fp64_inst_per_warp_cell"]), r["profile"]
+
+
+def alu_roofs(segments, march_ms, sm_mhz, inst_per_cell, fp64_per_cell):
+    """The march kernel against the hardware's fp64-pipe roof and against the issue roof of its own instruction
+    stream; both in segments/s at the SM clock measured during the run."""
+    slots = SM_COUNT * SCHEDULERS_PER_SM * sm_mhz * 1e6 * LANES      # lane-slots per second
+    ach = segments / (march_ms * 1e-3)
+    fp64_peak = slots / (FP64_PIPE_CYCLES_PER_WARP_INST * fp64_per_cell)
+    issue_peak = slots / inst_per_cell
+    return dict(achieved=ach, fp64_peak=fp64_peak, fp64_frac=ach / fp64_peak, issue_peak=issue_peak,
+                issue_frac=ach / issue_peak)
 
 
 def parse():
@@ -56,9 +86,13 @@ def parse():
     ap.add_argument("--timestep-myr", type=float, default=0.0,
                     help="time a whole RT timestep of this length (iterative RT<->ODE solve, nyxrt_timestep) instead of one RT step")
     ap.add_argument("--periodic", action="store_true", help="periodic box (default: BASELINE.json's open box)")
-    ap.add_argument("--graph-loop", action="store_true",
-                    help="time the production loop (one CUDA-graph launch per trace; no per-launch events, so the "
-                         "roofline's achieved figure then uses the loop time instead of the march launches' own)")
+    ap.add_argument("--graph-loop", action="store_true", help="(the default now; kept so that old commands still run)")
+    ap.add_argument("--profiling-loop", action="store_true",
+                    help="time the host-enqueued profiling loop (NYXRT_FLAG_LAUNCH_TIMING) instead of the production "
+                         "CUDA-graph loop for value / e2e, as rounds 1-2 did")
+    ap.add_argument("--profile-steps", type=int, default=1,
+                    help="steps of the separate profiling pass (per-launch CUDA events around every march launch) that "
+                         "feeds the roofline; 0: roofline from the loop time of the timed steps")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -257,27 +291,32 @@ def main():
     cfg, pos, L = make_workload(args, "cuda")
     nH, xHI = cfg["nH"], cfg["xHI"]
     fdt = "f32" if nH.dtype == torch.float32 else "f64"
-    params = dict(cfg["params"])
-    params["flags"] = 0 if args.graph_loop else nyxrt.FLAG_LAUNCH_TIMING    # per-launch events: what the roofline needs
-    tr = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], params, field_dtype=nH.dtype, max_sources=len(L),
-                      batch_rays=args.batch_rays, host_staging=not args.no_e2e, device=local,
-                      periodic=1 if args.periodic else 0)
-    if args.spectrum_teff > 0:
-        tr.set_spectrum(-20, 12, 8, nyxrt.nyxrt_blackbody_table(args.spectrum_teff, -20, 12, 8))
-        if args.tau_thin > 0:
-            tr.set_spectrum_thin(nyxrt.nyxrt_blackbody_thin_table(args.spectrum_teff, -20, 12, 8), args.tau_thin)
+    timed_flags = nyxrt.FLAG_LAUNCH_TIMING if args.profiling_loop else 0      # 0: the production CUDA-graph loop
+
+    def make_tracer(flags, host_staging):
+        params = dict(cfg["params"])
+        params["flags"] = flags
+        t = nyxrt.Tracer(cfg["shape"], cfg["dx_cm"], params, field_dtype=nH.dtype, max_sources=len(L),
+                         batch_rays=args.batch_rays, host_staging=host_staging, device=local,
+                         periodic=1 if args.periodic else 0)
+        if args.spectrum_teff > 0:
+            t.set_spectrum(-20, 12, 8, nyxrt.nyxrt_blackbody_table(args.spectrum_teff, -20, 12, 8))
+            if args.tau_thin > 0:
+                t.set_spectrum_thin(nyxrt.nyxrt_blackbody_thin_table(args.spectrum_teff, -20, 12, 8), args.tau_thin)
+        if args.shard:
+            t.set_shard(rank, world)
+        return t
+
+    tr = make_tracer(timed_flags, not args.no_e2e)
     gam = torch.empty(cfg["shape"], dtype=torch.float64, device="cuda")
     heat = torch.empty_like(gam)
     stream = torch.cuda.current_stream()
-
     photons = torch.empty_like(gam) if args.shard else None
-    if args.shard:
-        tr.set_shard(rank, world)
 
     class _TS:                                                     # timestep mode: the sum over the iterations
         pass
 
-    def step():
+    def step(tr):
         # one RT step: fields of this step -> absorber field, sources -> catalogue, ray loop, finalise
         if args.timestep_myr > 0:
             tr.set_sources(pos, L, stream)
@@ -290,7 +329,9 @@ def main():
             out.segments = ts.segments_total
             out.kernel_launches = ts.kernel_launches
             out.ms_march = st1.ms_march * ts.iterations           # per-launch events exist for the last trace only
+            out.ms_loop = st1.ms_loop * ts.iterations
             out.march_launches = st1.march_launches * ts.iterations
+            out.neighbour_deposits = st1.neighbour_deposits * ts.iterations
             out.timestep = dict(iterations=ts.iterations, converged=ts.converged, ms_rt=ts.ms_rt, ms_ode=ts.ms_ode,
                                 unconverged_cells=int(ts.unconverged_cells))
             return out
@@ -306,31 +347,37 @@ def main():
         return st_
 
     for _ in range(args.warmup):
-        st = step()
+        st = step(tr)
     barrier()
     clocks = ClockSampler(local)
     if rank == 0:
         clocks.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     seg = 0
-    nbr = 0
-    ms_march = 0.0
     launches = 0
-    march_launches = 0
+    prof = dict(seg=0, nbr=0, ms_march=0.0, march_launches=0, ms=0.0, steps=0, kind="")
     barrier()
     e0.record(stream)
     for _ in range(args.steps):
-        st = step()
+        st = step(tr)
         seg += st.segments
-        nbr += st.neighbour_deposits
-        ms_march += st.ms_march if not args.graph_loop else st.ms_loop
         launches += st.kernel_launches + 3            # + prep_fields, sum_partials, snap
-        march_launches += st.march_launches
+        if args.profiling_loop or args.profile_steps <= 0:
+            # no separate profiling pass: the march launches' own durations if this loop measures them, else the loop time
+            prof["seg"] += st.segments
+            prof["nbr"] += st.neighbour_deposits
+            prof["ms_march"] += st.ms_march if args.profiling_loop else st.ms_loop
+            prof["march_launches"] += st.march_launches
+            prof["steps"] += 1
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
     clk = clocks.stop() if rank == 0 else None
     ms = max_over_ranks(ms, "cuda")
+    if prof["steps"]:
+        prof["ms"] = ms
+        prof["kind"] = ("the timed steps (profiling loop)" if args.profiling_loop
+                        else "the timed steps; no per-launch events: the loop time stands in for the march launches' own")
     if args.timestep_myr > 0:
         args.no_e2e = True
     if args.shard:
@@ -364,30 +411,61 @@ def main():
                    checksum_gamma_sum=float(h_g.sum()))
         del h_nH, h_xHI, h_g, h_h
 
+    # ---- profiling pass for the roofline: the same step through the host-enqueued loop, which puts a CUDA-event pair
+    # around every march launch (NYXRT_FLAG_LAUNCH_TIMING).  Same kernels, same results; outside the timed region. ----
+    if not prof["steps"]:
+        tr.close()
+        tr = make_tracer(nyxrt.FLAG_LAUNCH_TIMING, False)
+        barrier()
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        for _ in range(args.profile_steps):
+            sp = step(tr)
+            prof["seg"] += sp.segments
+            prof["nbr"] += sp.neighbour_deposits
+            prof["ms_march"] += sp.ms_march
+            prof["march_launches"] += sp.march_launches
+            prof["steps"] += 1
+        p1.record(stream)
+        barrier()
+        prof["ms"] = p0.elapsed_time(p1)
+        prof["kind"] = "%d extra step(s) after the timed region, host-enqueued loop with per-launch events" % args.profile_steps
+
     if rank == 0:
         peak, peak_src = measured_peak()
+        pseg, pnbr, ms_march, march_launches = prof["seg"], prof["nbr"], prof["ms_march"], prof["march_launches"]
+        sm_mhz = float((clk or {}).get("sm_mhz") or 1965.0)
+        ipc, fpc, iprof = march_instruction_counts()
+        alu = alu_roofs(pseg, ms_march, sm_mhz, ipc, fpc)
+        avg_launch_ms = ms_march / max(march_launches, 1)
+        # Primary roof: the fp64 pipe.  ncu shows the kernel bound by instruction issue behind fp64 dependencies, with
+        # DRAM at 0.14 of its peak (profiles/r2_march_config5.md), so HBM is reported beside it, not as the bound.
+        roof = dict(bound="alu", kernel="march_kernel<3>", achieved=alu["achieved"], peak=alu["fp64_peak"],
+                    unit="segments/s", frac=alu["fp64_frac"], traffic=None,
+                    peak_source="148 SMs x 4 schedulers x %.0f MHz (median during the timed steps) x 32 lanes / (2 fp64-pipe "
+                                "cycles x %g fp64 warp instructions per warp-cell, profiles/march_instr.csv row %s)"
+                                % (sm_mhz, fpc, iprof),
+                    segments_per_launch=pseg / max(march_launches, 1), avg_launch_ms=avg_launch_ms,
+                    march_share_of_step=ms_march / max(prof["ms"], 1e-9), measured_on=prof["kind"],
+                    note="achieved = segments / sum of the march launches' durations (CUDA events around every launch on "
+                         "the launching stream); peak = the hardware's fp64-pipe roof for this kernel's counted fp64 "
+                         "instructions, all lanes busy and no stall")
+        roof["issue"] = dict(peak=alu["issue_peak"], frac=alu["issue_frac"], inst_per_warp_cell=ipc, unit="segments/s",
+                             note="issue-slot roof of the kernel's own instruction stream (one warp instruction per "
+                                  "scheduler per cycle); a leaner kernel raises this roof, the fp64 roof above it does not move")
+        # HBM, three ways: the contract's algorithmic bytes (48 / 64 B per segment), the same with the
+        # neighbour traffic counted instead of assumed, and the DRAM bytes ncu measured per launch
         bps = ALGO_BYTES_PER_SEGMENT[fdt]
-        ach = bps * seg / (ms_march * 1e-3) / 1e9          # algorithmic GB/s of the march launches alone
-        roof = dict(bound="hbm", kernel="march_kernel<3>", achieved=ach, peak=peak, unit="GB/s", frac=ach / peak,
-                    traffic=None, algorithmic_bytes_per_segment=bps, segments_per_launch=seg / max(march_launches, 1),
-                    avg_launch_ms=ms_march / max(march_launches, 1), march_share_of_step=ms_march / ms,
-                    peak_source=peak_src,
-                    note="achieved = %d B x segments / sum of march-launch durations (CUDA events around every "
-                         "launch on the launching stream); DRAM traffic per launch: see profiles/" % bps)
-        # the same with the neighbour traffic counted, not assumed: (2 field loads + 1 accumulator RMW) per segment
-        # and per neighbour deposit the library counted
+        ach = bps * pseg / (ms_march * 1e-3) / 1e9
         cb = ALGO_BYTES_CELL[fdt]
-        ach_x = cb * (seg + nbr) / (ms_march * 1e-3) / 1e9
-        roof["counted"] = dict(achieved=ach_x, frac=ach_x / peak, bytes_per_segment=cb * (seg + nbr) / max(seg, 1),
-                               neighbour_deposits_per_segment=nbr / max(seg, 1),
-                               note="%d B per segment + %d B per counted neighbour deposit" % (cb, cb))
-        sm_hz = 1e6 * float((clk or {}).get("sm_mhz") or 1965.0)
-        alu_peak = SM_COUNT * SCHEDULERS_PER_SM * sm_hz * LANES / ISSUE_CYCLES_PER_WARP_CELL
-        roof["alu"] = dict(bound="alu", achieved=seg / (ms_march * 1e-3), peak=alu_peak, unit="segments/s",
-                           frac=seg / (ms_march * 1e-3) / alu_peak,
-                           note="issue-slot roof of the march kernel: SMs x 4 schedulers x SM clock x 32 lanes / %d issue "
-                                "cycles per warp-cell (all lanes busy, no stall); the kernel is bound by this, not by HBM"
-                                % ISSUE_CYCLES_PER_WARP_CELL)
+        ach_x = cb * (pseg + pnbr) / (ms_march * 1e-3) / 1e9
+        roof["hbm"] = dict(peak=peak, unit="GB/s", peak_source=peak_src,
+                           algorithmic=dict(achieved=ach, frac=ach / peak, bytes_per_segment=bps,
+                                            note="%d B x segments / march time: the figure rounds 1-2 reported as roofline.frac" % bps),
+                           counted=dict(achieved=ach_x, frac=ach_x / peak, bytes_per_segment=cb * (pseg + pnbr) / max(pseg, 1),
+                                        neighbour_deposits_per_segment=pnbr / max(pseg, 1),
+                                        note="%d B per segment + %d B per counted neighbour deposit" % (cb, cb)),
+                           measured=None)
         # DRAM bytes per march launch measured by ncu on THIS workload (profiles/march_traffic.csv, one row per
         # captured launch; profiles/march_traffic.md has the commands); null when no capture matches the run
         tfile = os.path.join(ROOT, "profiles", "march_traffic.csv")
@@ -406,12 +484,20 @@ def main():
                     roof["traffic"] = sum(tb) / len(tb)
                     roof["traffic_note"] = ("mean dram__bytes_read.sum + dram__bytes_write.sum of %d captured march launches "
                                             "of this workload (ncu --set full, mean %.2f ms under ncu)" % (len(tb), sum(tm) / len(tm)))
+                    dram = sum(b / (1e-3 * t) for b, t in zip(tb, tm)) / len(tb) / 1e9
+                    roof["hbm"]["measured"] = dict(achieved=dram, frac=dram / peak,
+                                                   note="DRAM bytes / duration of the same captured launches (under ncu)")
+                    iu = [float(r["issue_active_pct"]) / 100.0 * float(r["active_threads_per_inst"]) / LANES for r in rows]
+                    roof["issue"]["issue_util_measured"] = sum(iu) / len(iu)
+                    roof["issue"]["issue_util_note"] = "ncu: issue slots busy x active threads per instruction / 32, same launches"
             except (ValueError, OSError, KeyError):
                 pass
         cpu = None
         if not args.no_cpu:
             cpu = oracle_sample(cfg, pos, L, args.cpu_seconds)
             cpu.pop("segments"); cpu.pop("seconds")
+        graph = "one CUDA-graph launch per trace (WHILE node over sched -> emit -> march): the production path"
+        hostl = "host-enqueued launches with a CUDA-event pair around every march launch (NYXRT_FLAG_LAUNCH_TIMING)"
         out = dict(metric=METRIC, value=value, unit="segments/s", n_gpus=world, steps=args.steps, warmup=args.warmup,
                    ms_per_step=ms / args.steps, higher_is_better=True, scaling="strong" if args.shard else "weak",
                    vs_baseline=None, dtype="f64", data="synthetic",
@@ -425,9 +511,11 @@ def main():
                                spectrum=("black body %g K, tau_0 table 2^-20..2^12, 256 nodes per octave%s" % (
                                    args.spectrum_teff, ", thin table below dtau_0 = %g" % args.tau_thin if args.tau_thin > 0 else ""))
                                if args.spectrum_teff > 0 else "monochromatic"),
-                   loop="one CUDA-graph launch per trace (WHILE node over sched -> emit -> march)" if args.graph_loop
-                   else "host-enqueued launches with a CUDA-event pair around every march launch (NYXRT_FLAG_LAUNCH_TIMING)",
-                   rt_step_ms=ms / args.steps, march_ms_per_step=ms_march / args.steps,
+                   loop=hostl if args.profiling_loop else graph,
+                   rt_step_ms=ms / args.steps,
+                   profiling_pass=dict(loop=hostl if (args.profiling_loop or args.profile_steps > 0) else graph,
+                                       steps=prof["steps"], ms_per_step=prof["ms"] / max(prof["steps"], 1),
+                                       march_ms_per_step=ms_march / max(prof["steps"], 1), measured_on=prof["kind"]),
                    gpu_launches=int(launches), clocks=clk, e2e=e2e, roofline=roof, cpu_baseline=cpu,
                    stats=dict(iterations=int(st.iterations), peak_pool_rays=int(st.peak_pool_rays),
                               ms_sources=st.ms_sources, ms_loop=st.ms_loop, ms_finalise=st.ms_finalise,

@@ -33,8 +33,10 @@
  * Gamma = sigma Ndot exp(-tau) / (4 pi R^2) (Eq. 1 with V_shell); Stroemgren I-front, Eq. 10-11
  * with Table 1 Test A; Eq. 5-8 special cases; split radii from Eq. 4;
  * brute-force O(N^2)+DFS merge.  Parity UNPINNED by the paper (no printed values): the bubble
- * sample pattern and the merge defaults (PAPER.md:315-333 leave them to the user), and the
- * figures 3, 4, 8c.
+ * sample pattern and the merge defaults (PAPER.md:315-333 leave them to the user), the
+ * figures 3, 4, 8c, and the reading of footnote 3 taken for thin segments -- the
+ * thin table evaluated at the segment's midpoint and the neighbour's share taken from it, R41-R42:
+ * T itself, the thin form's accuracy and the budget are pinned, the choice of reading is not.
  */
 #include <math.h>
 #include <stdint.h>

@@ -49,3 +49,18 @@ def test_reference_arm_other_ranks_exit_quietly():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_alu_roofs_come_from_the_committed_instruction_counts():
+    """The march kernel's roofs are derived from profiles/march_instr.csv (last row), not from a constant in bench.py:
+    148 SMs x 4 schedulers x clock x 32 lanes / cycles per warp-cell, 2 fp64-pipe cycles per fp64 warp instruction."""
+    sys.path.insert(0, ROOT)
+    import bench
+    ipc, fpc, prof = bench.march_instruction_counts()
+    assert 100 <= ipc <= 400 and 40 <= fpc < ipc and prof.endswith(".md")
+    assert os.path.exists(os.path.join(ROOT, "profiles", prof))
+    r = bench.alu_roofs(segments=1.0e12, march_ms=10_000.0, sm_mhz=1965.0, inst_per_cell=200.0, fp64_per_cell=80.0)
+    slots = 148 * 4 * 1965e6 * 32
+    assert abs(r["achieved"] - 1.0e11) < 1.0
+    assert abs(r["fp64_peak"] - slots / 160.0) < 1.0 and abs(r["issue_peak"] - slots / 200.0) < 1.0
+    assert abs(r["fp64_frac"] - 1.0e11 * 160.0 / slots) < 1e-12 and r["issue_frac"] > r["fp64_frac"]
