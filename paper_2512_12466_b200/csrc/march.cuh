@@ -211,6 +211,20 @@ __device__ __forceinline__ double lut_t(const MarchArgs &A, double tau) {
     return fma(frac, t1 - t0, t0);
 }
 
+// Both tables through one gather pair (LUT == 2): `thin` picks T (and its edge rule) or Q; the value is lut_t's or
+// lut_q's, bit for bit.  Lanes of a warp that disagree on `thin` then still share one lookup instead of running
+// the two routines one after the other.
+__device__ __forceinline__ double lut_qt(const MarchArgs &A, double x, bool thin) {
+    if (!(x >= A.lut_t_lo)) return thin ? A.lut_t_first : (x > 0.0 ? A.lut_q_first * (x * A.lut_inv_t_lo) : 0.0);
+    if (x >= A.lut_t_hi) return thin ? A.lut_t_last : A.lut_q_last;
+    const long long bits = __double_as_longlong(x);
+    const long long k = (bits >> A.lut_fb) - A.lut_k0;
+    const double frac = (double)(bits & A.lut_fmask) * A.lut_fscale;
+    const double *__restrict__ tab = thin ? A.lut_t : A.lut_q;
+    const double v0 = __ldg(tab + k), v1 = __ldg(tab + k + 1);
+    return fma(frac, v1 - v0, v0);
+}
+
 // One ray-cell segment, described by the geometry stage and consumed by the physics stage one iteration
 // later (so that its two absorber gathers have a whole iteration to arrive).
 template <typename IDX>
@@ -289,6 +303,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
     // cell to be traversed, while two of SA / SB / SC hold the segments whose absorber loads are in flight.
     bool has = false;
     double s = 0.0, tau = 0.0, N = 0.0;
+    double q_tau = -1.0;               // LUT == 2: Q(tau) left by the last thick segment (Q >= 0; -1: look it up)
     double od0 = 0, od1 = 0, od2 = 0, sx0 = 0, sx1 = 0, sx2 = 0;
     IDX c = 0;                                     // cell (padded linear index)
     unsigned long long cnt = 0;                    // periodic box: steps left to the faces (3 x 21 bits)
@@ -393,8 +408,15 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 const double dtau = (fabs(D.a_c) * sdx) * D.ds;
                 double pm, left, dN;
                 if constexpr (LUT == 2) {
-                    const double frac = dtau < A.tau_thin ? dtau * lut_t(A, tau + 0.5 * dtau)
-                                                           : lut_q(A, tau + dtau) - lut_q(A, tau);
+                    // thin: dtau T(tau + dtau/2); thick: Q(tau + dtau) - Q(tau), where Q(tau) is the previous thick
+                    // segment's Q(tau + dtau) -- `tau` is that very double, so the carried value has the bits a second
+                    // lookup would return; it is looked up only after a thin segment or a pop
+                    const bool thin = dtau < A.tau_thin;
+                    const double v = lut_qt(A, thin ? tau + 0.5 * dtau : tau + dtau, thin);
+                    double q_a = q_tau;
+                    if (!thin && q_a < 0.0) q_a = lut_q(A, tau);
+                    const double frac = thin ? dtau * v : v - q_a;
+                    q_tau = thin ? -1.0 : v;
                     dN = T.w.v[threadIdx.x] * frac;
                     left = N - dN;
                     pm = 0.0;
@@ -565,6 +587,7 @@ __global__ void __launch_bounds__(MARCH_THREADS, MARCH_MIN_BLOCKS) march_kernel(
                 const int e = qhead + rank;
                 T.key[threadIdx.x] = Q.key[wid][e];
                 s = Q.s[wid][e]; tau = Q.tau[wid][e]; N = Q.N[wid][e];
+                q_tau = -1.0;
                 if constexpr (LUT == 1) { T.w.v[threadIdx.x] = N; N = lut_q(A, tau); }
                 if constexpr (LUT == 2)                                           // the share L / (12 4^l)
                     T.w.v[threadIdx.x] = A.cat_L[key_src(Q.key[wid][e])] / (12.0 * (double)(1ll << (2 * level)));
