@@ -134,3 +134,42 @@ def test_bad_arguments():
     with pytest.raises(nyxrt.NyxrtError):
         tr.timestep(nyxrt.make_ode(0.0), f, f)
     tr.close()
+
+
+def test_correction_modes_stromgren_fig8c(O):
+    """What the correction-mode switch is for (without the secondary correction the photons a
+    ray cannot give to its own cell are lost, and "squaring f_c can increase photon loss"; Fig. 8c): Stroemgren Test A
+    (Eq. 10-11) through nyxrt_timestep for every geom_mode, ten 1 Myr steps from a
+    neutral box, the ionised volume's radius r_I(t) against Eq. 11 at every step.  GPU against the oracle by the
+    parity rule at every step of every mode; then the shape: modes 0 (no correction), 2 (Eq. 5-6) and 3 (Eq. 7-8;
+    the same as 2 here, the n_th rule is inactive in a uniform box) conserve photons and follow Eq. 11 to 2 %;
+    mode 1 (Eq. 5 alone) loses about a tenth of the photons and lags; mode 4 (f_c squared, [59]) loses about twice
+    as many and lags further.  The table in BASELINE.md section 4 is this test's output."""
+    cfg = synth.make(1)
+    dx, nH0, Nd, aB = cfg["dx_cm"], 1e-3, 5e48, 2.59e-13
+    rs = (3 * Nd / (4 * math.pi * aB * nH0 ** 2)) ** (1 / 3)
+    trec = 1.0 / (aB * nH0)
+    ratio, lost = {}, {}
+    for mode in (0, 1, 2, 3, 4):
+        c = dict(cfg)
+        c["params"] = dict(cfg["params"], geom_mode=mode)
+        y, t, ratio[mode], lost[mode] = cfg["xHI"].double(), 0.0, [], []
+        for k in range(10):
+            c["xHI"] = y
+            rg, ro = run_both(O, c, 1.0 * MYR)
+            compare(rg, ro)
+            assert abs(rg[4].photons_lost - ro[4].photons_lost) <= 1e-11 * ro[4].photons_emitted
+            y = torch.from_numpy(rg[0])
+            t += 1.0 * MYR
+            rn = (3 * float((1.0 - y).sum()) * dx ** 3 / (4 * math.pi)) ** (1 / 3)
+            ratio[mode].append(rn / (rs * (1 - math.exp(-t / trec)) ** (1 / 3)))
+            lost[mode].append(rg[4].photons_lost / rg[4].photons_emitted)
+        print("geom_mode %d: r_I / Eq. 11 at 1..10 Myr = %s; photons lost in the last trace %.4f"
+              % (mode, " ".join("%.4f" % v for v in ratio[mode]), lost[mode][-1]))
+    for mode in (0, 2, 3):
+        assert all(abs(v - 1.0) < 0.02 for v in ratio[mode]) and max(lost[mode]) == 0.0, mode
+    assert all(abs(a - b) <= 1e-9 for a, b in zip(ratio[2], ratio[3]))
+    for k in range(10):
+        assert ratio[4][k] < ratio[1][k] < ratio[2][k] - 0.03, k
+        assert lost[4][k] > lost[1][k] > 0.02, k
+    assert 0.93 < ratio[1][-1] < 0.97 and 0.88 < ratio[4][-1] < 0.93 and lost[4][-1] > 1.5 * lost[1][-1] > 0.05
