@@ -9,8 +9,9 @@ import pytest
 
 
 def ang2pix_nest(level, v):
-    """Inverse map, written from the HEALPix paper's projection equations (equatorial: cylindrical
-    equal-area; polar caps: Collignon), not from the oracle."""
+    """Inverse map (vector -> nested pixel) after the HEALPix library's `loc2pix` routine, the standard
+    statement of Gorski et al.'s projection (equatorial: cylindrical equal-area; polar caps: Collignon): a
+    restated public algorithm, used here only as a pin.  It shares nothing with the oracle's pix -> vector code."""
     ns = 1 << level
     x, y, z = v
     za = abs(z)
